@@ -1,0 +1,149 @@
+/*
+ * swb200.h -- C-ABI of libswb200.so: Swendsen-Wang and Wolff cluster updates of the 2D nearest-neighbour
+ * Ising / q-state Potts model on a periodic L x L square lattice, hand-written CUDA for sm_100a (B200).
+ *
+ * Method: M. Weigel, "Connected component identification and cluster update on GPU", arXiv:1105.5804.
+ * "P:NN" = line NN of the paper text; "S:8x" = SURVEY.md section 8(x); DESIGN.md lists every
+ * reading of the paper taken here.
+ *
+ * Conventions (S:8b, S:8c):
+ *   - site i = y*L + x, x,y in [0,L); east(i) = (x+1 mod L, y); north(i) = (x, y+1 mod L)   (P:66 periodic
+ *     square lattice; Fig. 1: site 0 bottom-left).
+ *   - q = 2: Ising convention, spins int8 in {+1,-1} (state k=0 -> +1, k=1 -> -1), bond probability
+ *     p = 1 - exp(-2 beta) (BASELINE.json configs), beta_c = ln(1+sqrt 2)/2.
+ *     3 <= q <= 8: Potts delta convention (Eq. 1), spins uint8 in [0,q), p = 1 - exp(-beta).  J = 1.
+ *   - random numbers: stateless Philox4x32-10, key = (seed low 32, seed high 32), counter
+ *     (c0, t low 32, t high 32, domain) with domains INIT=0, BOND=1, FLIP=2, WSEED=3; t is the step counter,
+ *     starting at 0 and increased by one per SW sweep or Wolff step (S:8c.2).  The paper's per-thread LCGs
+ *      make results depend on the thread layout and are replaced (reading 5).
+ *   - labels are canonical: labels[i] = the minimum site index of i's cluster (BASELINE.json north_star (3)).
+ *   - packed bonds: byte b holds sites 4b..4b+3; site j uses bit 2(j&3) (east bond) and 2(j&3)+1 (north bond).
+ *
+ * Memory: every `d_` pointer is DEVICE memory owned by the caller (e.g. a torch tensor), 16-byte aligned, alive
+ * for as long as it is bound.  The handle owns only host state and never frees caller memory.  `h_` pointers
+ * are HOST memory.  `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  All
+ * kernels are enqueued on that stream; a function is asynchronous unless it says "synchronises".
+ *
+ * Errors: every function returns SW_OK (0) or a negative code; nothing throws, aborts or prints.
+ */
+#ifndef SWB200_H
+#define SWB200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    SW_OK      = 0,
+    SW_EINVAL  = -1,  /* bad argument: L<4, L%4!=0, L>32768, q outside [2,8], beta not finite or <0, NULL or
+                         misaligned pointer, workspace too small, n<0                                      */
+    SW_ESTATE  = -2,  /* handle not bound (sw_bind not called), or d_bonds needed but bound as NULL        */
+    SW_ECUDA   = -3,  /* a CUDA runtime call or kernel launch failed; text via sw_strerror / sw_last_cuda_error */
+    SW_ENOMEM  = -4   /* host allocation failed                                                          */
+};
+
+typedef struct sw_handle sw_handle;   /* opaque; host-side state only */
+
+/* Observables (S:8a a6, a9).  Spin part: Eq. 1.  Cluster part refers to the labelling performed by the
+ * LAST sw_sweep / wolff_step / sw_label on this handle (reading 13); zero if none happened yet. */
+typedef struct {
+    int64_t  sat_bonds;        /* number of the 2N bonds whose end spins are equal                            */
+    int64_t  energy;           /* q=2: -sum_<ij> s_i s_j = -(2 sat - 2N);  q>2: -sat  (Eq. 1 with J=1)    */
+    int64_t  magnetisation;    /* q=2: sum_i s_i;  q>2: q * max_k n_k - N                                     */
+    int64_t  state_count[8];   /* n_k = number of sites in state k, k < q                                     */
+    int64_t  n_clusters;       /* #{ i : labels[i] == i }                                                     */
+    int64_t  n_active_bonds;   /* bonds activated in the last sweep / step (0 after sw_label)                 */
+    int64_t  max_cluster;      /* size of the largest cluster                                                 */
+    uint64_t sum_sq_cluster;   /* sum over clusters of size^2 (FK estimator of N^2 <m^2>)                     */
+    uint64_t counter;          /* step counter t after the last sweep / step                                  */
+} sw_obs;
+
+/* Cluster statistics of a canonical labelling (S:8a a9; BASELINE.json config 4 "cluster-size histogram"). */
+typedef struct {
+    int64_t  n_clusters;
+    int64_t  max_cluster;
+    uint64_t sum_sq_cluster;
+    int64_t  hist32[32];       /* hist32[b] = number of clusters with 2^b <= size < 2^(b+1)                   */
+} sw_cstats;
+
+/* Create a handle for an L x L lattice of q-state spins at inverse temperature beta with RNG seed `seed`
+ * (BASELINE.json north_star "sw_create(L,q,beta,seed)").  The bond threshold is T = floor((1-exp(-K beta)) 2^32)
+ * in IEEE double on the host, K = 2 for q=2, K = 1 otherwise (S:8c.4); a bond between equal spins is activated
+ * iff its 32-bit draw is < T (P:53 step 1, Eq. 7).  Requires 4 <= L <= 32768, L % 4 == 0, 2 <= q <= 8,
+ * beta finite and >= 0.  The step counter starts at 0.  No device memory is allocated. */
+int sw_create(sw_handle** out, int32_t L, int32_t q, double beta, uint64_t seed);
+int sw_destroy(sw_handle* h);
+
+/* Bytes of device workspace sw_bind needs for an L x L lattice (seam bond bytes, int32 cluster-size scratch,
+ * accumulators).  0 if L or q is invalid. */
+size_t sw_workspace_bytes(int32_t L, int32_t q);
+
+/* Bind caller-owned device buffers: d_spins N bytes (int8 for q=2, uint8 for q>2), d_labels N int32,
+ * d_bonds N/4 bytes of packed bonds or NULL (only sw_activate and sw_label(d_bonds=NULL) need it),
+ * d_work >= sw_workspace_bytes(L,q) bytes.  Zeroes the accumulators in d_work on `stream`. */
+int sw_bind(sw_handle* h, void* d_spins, int32_t* d_labels, uint8_t* d_bonds, void* d_work, size_t work_bytes,
+            void* stream);
+
+/* Threshold override (percolation, BASELINE.json config 4; tests) and step-counter access (checkpoint /
+ * resume: the whole state is (spins, t), S:5). */
+int sw_set_threshold(sw_handle* h, uint32_t T);
+int sw_get_threshold(const sw_handle* h, uint32_t* T);
+int sw_set_counter(sw_handle* h, uint64_t t);
+int sw_get_counter(const sw_handle* h, uint64_t* t);
+
+/* Initialise d_spins (S:8c.8): mode 0 = cold (all k=0, i.e. +1 for q=2); mode 1 = random,
+ * k_i = (PHILOX(seed; i>>2, 0, 0, INIT)[i&3] * q) >> 32.  Does not change the counter. */
+int sw_init_spins(sw_handle* h, int mode, void* stream);
+
+/* n Swendsen-Wang sweeps (P:51-55 steps 1-3), asynchronous; t += n.  Each sweep at counter t:
+ *   1. bond activation (S:8c.3-4): n(i,d) = [s_i == s_nbr(i,d)] and [PHILOX(seed; i>>1, t, BOND)[2(i&1)+d] < T]
+ *   2. labelling: d_labels[i] = min site index of i's connected component in the activated-bond graph
+ *   3. flip: every cluster with root r takes state k_r = (PHILOX(seed; r, t, FLIP)[0] * q) >> 32 (P:55 step 3)
+ * After return (and stream completion) d_spins holds the new configuration and d_labels the canonical labels of
+ * the last sweep's bond graph. */
+int sw_sweep(sw_handle* h, int64_t n, void* stream);
+
+/* Write the packed bonds of step t (the current counter, not advanced) for the current spins into the bound
+ * d_bonds ("bond array"; S:8a a1).  SW_ESTATE if d_bonds was bound as NULL. */
+int sw_activate(sw_handle* h, void* stream);
+
+/* Connected-component labelling of an arbitrary packed bond array on the L x L torus
+ * (BASELINE.json north_star "sw_label(bonds->labels)"; P:54 step 2; config 4 percolation):
+ * d_labels_out[i] = min site index of i's component.  d_bonds_in == NULL uses the bound d_bonds,
+ * d_labels_out == NULL the bound d_labels.  Does not touch spins or the counter. */
+int sw_label(sw_handle* h, const uint8_t* d_bonds_in, int32_t* d_labels_out, void* stream);
+
+/* Cluster statistics of canonical labels (d_labels_in == NULL: the bound d_labels).  Synchronises `stream`. */
+int sw_cluster_stats(sw_handle* h, const int32_t* d_labels_in, sw_cstats* h_out, void* stream);
+
+/* n Wolff single-cluster steps, q = 2 only (SW_EINVAL otherwise; reading 8); t += n.
+ * Step at counter t (S:8c.9): seed site i0 = (PHILOX(seed; 0, t, WSEED)[0] * N) >> 32; C = component of i0 in the
+ * bond graph of step t on the pre-step spins; s_i -> -s_i for i in C.  Realised as "decompose the whole lattice,
+ * flip one cluster" (P:334 option (a)).  h_sizes: NULL, or a HOST array of n int64 that receives |C| of every
+ * step -- in that case the call synchronises `stream` before returning. */
+int wolff_step(sw_handle* h, int64_t n, int64_t* h_sizes, void* stream);
+
+/* Energy, magnetisation, state counts of the current spins and cluster statistics of the current labels, all in
+ * int64 (S:8a a6).  Synchronises `stream`. */
+int sw_observables(sw_handle* h, sw_obs* h_out, void* stream);
+
+/* Host-buffer convenience for end-to-end use: copy h_spins_in (N bytes, may be NULL to keep the device state)
+ * to the device, run n sweeps, copy spins back to h_spins_out (may be NULL) and labels to h_labels_out (may be
+ * NULL), fill h_obs (may be NULL).  Synchronises `stream`. */
+int sw_sweep_host(sw_handle* h, const void* h_spins_in, int64_t n, void* h_spins_out, int32_t* h_labels_out,
+                  sw_obs* h_obs, void* stream);
+
+/* Number of kernels this handle has launched so far (for bench.py's gpu_launches). */
+int sw_launch_count(const sw_handle* h, uint64_t* n);
+
+const char* sw_strerror(int code);
+/* Text of the last CUDA error seen by this handle ("" if none). */
+const char* sw_last_cuda_error(const sw_handle* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SWB200_H */

@@ -1,0 +1,213 @@
+"""Thin ctypes binding of libswb200.so (include/swb200.h): same names, argument marshalling only.
+
+torch is used for device memory and streams only.  If the shared library is missing or cannot be loaded this
+module raises -- there is no CPU fallback and nothing here imports ``oracle``.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libswb200.so")
+
+SW_OK, SW_EINVAL, SW_ESTATE, SW_ECUDA, SW_ENOMEM = 0, -1, -2, -3, -4
+
+# every symbol include/swb200.h declares (tests check that the library exports all of them)
+SYMBOLS = [
+    "sw_create", "sw_destroy", "sw_workspace_bytes", "sw_bind", "sw_set_threshold", "sw_get_threshold",
+    "sw_set_counter", "sw_get_counter", "sw_init_spins", "sw_sweep", "sw_activate", "sw_label",
+    "sw_cluster_stats", "wolff_step", "sw_observables", "sw_sweep_host", "sw_launch_count", "sw_strerror",
+    "sw_last_cuda_error",
+]
+
+
+class sw_obs(C.Structure):
+    _fields_ = [("sat_bonds", C.c_int64), ("energy", C.c_int64), ("magnetisation", C.c_int64),
+                ("state_count", C.c_int64 * 8), ("n_clusters", C.c_int64), ("n_active_bonds", C.c_int64),
+                ("max_cluster", C.c_int64), ("sum_sq_cluster", C.c_uint64), ("counter", C.c_uint64)]
+
+    def as_dict(self):
+        return {"sat_bonds": self.sat_bonds, "energy": self.energy, "magnetisation": self.magnetisation,
+                "state_count": list(self.state_count), "n_clusters": self.n_clusters,
+                "n_active_bonds": self.n_active_bonds, "max_cluster": self.max_cluster,
+                "sum_sq_cluster": self.sum_sq_cluster, "counter": self.counter}
+
+
+class sw_cstats(C.Structure):
+    _fields_ = [("n_clusters", C.c_int64), ("max_cluster", C.c_int64), ("sum_sq_cluster", C.c_uint64),
+                ("hist32", C.c_int64 * 32)]
+
+    def as_dict(self):
+        return {"n_clusters": self.n_clusters, "max_cluster": self.max_cluster,
+                "sum_sq_cluster": self.sum_sq_cluster, "hist32": list(self.hist32)}
+
+
+_lib = None
+
+
+def lib():
+    """Load libswb200.so (building it first if the sources are newer and nvcc is present)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        from . import build as _build
+        _build.build()                                    # raises if nvcc is missing
+    L = C.CDLL(LIB_PATH)
+    vp, i32, i64, u32, u64 = C.c_void_p, C.c_int32, C.c_int64, C.c_uint32, C.c_uint64
+    L.sw_create.argtypes = [C.POINTER(vp), i32, i32, C.c_double, u64]
+    L.sw_destroy.argtypes = [vp]
+    L.sw_workspace_bytes.argtypes = [i32, i32]
+    L.sw_workspace_bytes.restype = C.c_size_t
+    L.sw_bind.argtypes = [vp, vp, vp, vp, vp, C.c_size_t, vp]
+    L.sw_set_threshold.argtypes = [vp, u32]
+    L.sw_get_threshold.argtypes = [vp, C.POINTER(u32)]
+    L.sw_set_counter.argtypes = [vp, u64]
+    L.sw_get_counter.argtypes = [vp, C.POINTER(u64)]
+    L.sw_init_spins.argtypes = [vp, C.c_int, vp]
+    L.sw_sweep.argtypes = [vp, i64, vp]
+    L.sw_activate.argtypes = [vp, vp]
+    L.sw_label.argtypes = [vp, vp, vp, vp]
+    L.sw_cluster_stats.argtypes = [vp, vp, C.POINTER(sw_cstats), vp]
+    L.wolff_step.argtypes = [vp, i64, C.POINTER(i64), vp]
+    L.sw_observables.argtypes = [vp, C.POINTER(sw_obs), vp]
+    L.sw_sweep_host.argtypes = [vp, vp, i64, vp, vp, C.POINTER(sw_obs), vp]
+    L.sw_launch_count.argtypes = [vp, C.POINTER(u64)]
+    L.sw_strerror.argtypes = [C.c_int]
+    L.sw_strerror.restype = C.c_char_p
+    L.sw_last_cuda_error.argtypes = [vp]
+    L.sw_last_cuda_error.restype = C.c_char_p
+    for name in SYMBOLS:
+        if name not in ("sw_workspace_bytes", "sw_strerror", "sw_last_cuda_error"):
+            getattr(L, name).restype = C.c_int
+    _lib = L
+    return L
+
+
+class SwError(RuntimeError):
+    def __init__(self, code, detail=""):
+        self.code = code
+        msg = lib().sw_strerror(code).decode()
+        super().__init__("swb200: %s (%d)%s" % (msg, code, (": " + detail) if detail else ""))
+
+
+class Lattice:
+    """One bound sw_handle plus the torch tensors it is bound to (device memory only; no arithmetic here)."""
+
+    def __init__(self, L: int, q: int, beta: float, seed: int, device="cuda:0", with_bonds: bool = False):
+        import torch
+        self._torch = torch
+        self._h = C.c_void_p()
+        self._lib = lib()
+        rc = self._lib.sw_create(C.byref(self._h), L, q, beta, seed)
+        if rc != SW_OK:
+            raise SwError(rc)
+        self.L, self.q, self.N = L, q, L * L
+        self.device = torch.device(device)
+        if self.device.type != "cuda":
+            raise RuntimeError("swb200 needs a CUDA device; there is no CPU path")
+        self.spins = torch.empty(self.N, dtype=torch.int8, device=self.device)
+        self.labels = torch.empty(self.N, dtype=torch.int32, device=self.device)
+        self.bonds = torch.empty(self.N // 4, dtype=torch.uint8, device=self.device) if with_bonds else None
+        wb = self._lib.sw_workspace_bytes(L, q)
+        self.work = torch.empty(wb, dtype=torch.uint8, device=self.device)
+        self._check(self._lib.sw_bind(self._h, self.spins.data_ptr(), self.labels.data_ptr(),
+                                      self.bonds.data_ptr() if with_bonds else None, self.work.data_ptr(), wb,
+                                      self._stream()))
+
+    # -- helpers ------------------------------------------------------------------------------------------
+    def _stream(self):
+        return C.c_void_p(self._torch.cuda.current_stream(self.device).cuda_stream)
+
+    def _check(self, rc):
+        if rc != SW_OK:
+            raise SwError(rc, self._lib.sw_last_cuda_error(self._h).decode() if rc == SW_ECUDA else "")
+
+    def close(self):
+        if self._h:
+            self._torch.cuda.synchronize(self.device)
+            self._lib.sw_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- the C-ABI, one method per entry point ---------------------------------------------------------------
+    def set_threshold(self, T: int):
+        self._check(self._lib.sw_set_threshold(self._h, T))
+
+    def get_threshold(self) -> int:
+        v = C.c_uint32()
+        self._check(self._lib.sw_get_threshold(self._h, C.byref(v)))
+        return v.value
+
+    def set_counter(self, t: int):
+        self._check(self._lib.sw_set_counter(self._h, t))
+
+    def get_counter(self) -> int:
+        v = C.c_uint64()
+        self._check(self._lib.sw_get_counter(self._h, C.byref(v)))
+        return v.value
+
+    def init_spins(self, mode: int):
+        self._check(self._lib.sw_init_spins(self._h, mode, self._stream()))
+
+    def sweep(self, n: int = 1):
+        self._check(self._lib.sw_sweep(self._h, n, self._stream()))
+
+    def activate(self):
+        self._check(self._lib.sw_activate(self._h, self._stream()))
+
+    def label(self, bonds=None, labels_out=None):
+        self._check(self._lib.sw_label(self._h, bonds.data_ptr() if bonds is not None else None,
+                                       labels_out.data_ptr() if labels_out is not None else None, self._stream()))
+
+    def cluster_stats(self, labels=None) -> dict:
+        out = sw_cstats()
+        self._check(self._lib.sw_cluster_stats(self._h, labels.data_ptr() if labels is not None else None,
+                                               C.byref(out), self._stream()))
+        return out.as_dict()
+
+    def wolff_step(self, n: int = 1, want_sizes: bool = True):
+        if want_sizes:
+            sizes = (C.c_int64 * n)()
+            self._check(self._lib.wolff_step(self._h, n, sizes, self._stream()))
+            return list(sizes)
+        self._check(self._lib.wolff_step(self._h, n, None, self._stream()))
+        return None
+
+    def observables(self) -> dict:
+        out = sw_obs()
+        self._check(self._lib.sw_observables(self._h, C.byref(out), self._stream()))
+        return out.as_dict()
+
+    def sweep_host(self, h_spins_in, n: int, h_spins_out=None, h_labels_out=None, want_obs: bool = True):
+        """Host-buffer end-to-end call: torch CPU tensors (ideally pinned) in and out."""
+        out = sw_obs()
+        self._check(self._lib.sw_sweep_host(
+            self._h, h_spins_in.data_ptr() if h_spins_in is not None else None, n,
+            h_spins_out.data_ptr() if h_spins_out is not None else None,
+            h_labels_out.data_ptr() if h_labels_out is not None else None,
+            C.byref(out) if want_obs else None, self._stream()))
+        return out.as_dict() if want_obs else None
+
+    def launch_count(self) -> int:
+        v = C.c_uint64()
+        self._check(self._lib.sw_launch_count(self._h, C.byref(v)))
+        return v.value
+
+    # -- convenience (copies only) -------------------------------------------------------------------------
+    def set_spins(self, host_array):
+        t = self._torch.from_numpy(host_array).view(self._torch.int8)
+        self.spins.copy_(t.to(self.device))
+
+    def spins_host(self):
+        return self.spins.cpu().numpy()
+
+    def labels_host(self):
+        return self.labels.cpu().numpy()

@@ -1,0 +1,87 @@
+// common.cuh -- lattice parameters, Philox4x32-10 and small device helpers shared by the sm_100a kernels.
+// Part of libswb200 (include/swb200.h).  Shares nothing with oracle/.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace swb {
+
+// Tile of the one-level decomposition ("tiles of B_x x B_y spins", P:84 B_x >> B_y for coalescing).
+// One CTA of 256 threads labels a TW x TH tile held in shared memory: lane -> 4 consecutive columns (one 32-bit
+// word of int8 spins, one 128-bit vector of int32 labels), warp -> TH/8 consecutive rows.
+constexpr int TW = 128;
+constexpr int TH = 64;
+constexpr int NTHREADS = 256;
+constexpr int NWARPS = NTHREADS / 32;
+constexpr int ROWS_PER_WARP = TH / NWARPS;
+
+enum : uint32_t { DOM_INIT = 0, DOM_BOND = 1, DOM_FLIP = 2, DOM_WSEED = 3 };
+
+// Everything a kernel needs to know about the lattice and the random stream; passed by value (constant bank).
+struct Params {
+    int32_t  L;          // edge length, multiple of 4
+    int32_t  N;          // L*L <= 2^30
+    int32_t  logL;       // log2(L) if L is a power of two, else -1
+    int32_t  q;          // number of Potts states (2 = Ising storage +-1)
+    int32_t  ntx, nty;   // number of tile columns / rows
+    uint32_t T;          // bond threshold floor(p 2^32)
+    uint32_t t_lo, t_hi; // step counter
+    uint64_t divL;       // ceil(2^40 / L): d / L == (d * divL) >> 40 for d < 2^24
+    uint32_t k0[10];     // Philox round keys: k0[r] = seed_lo + r * 0x9E3779B9
+    uint32_t k1[10];     //                    k1[r] = seed_hi + r * 0xBB67AE85
+};
+
+// Philox4x32-10 (Salmon et al., SC'11).  c1,c2,c3 are warp-uniform in every use here (step counter and domain).
+__device__ __forceinline__ void philox4x32_10(const Params& p, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                              uint32_t& w0, uint32_t& w1, uint32_t& w2, uint32_t& w3)
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        const uint32_t n0 = hi1 ^ c1 ^ p.k0[r];
+        const uint32_t n2 = hi0 ^ c3 ^ p.k1[r];
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+    }
+    w0 = c0; w1 = c1; w2 = c2; w3 = c3;
+}
+
+// d / L for 0 <= d < 2^24 (tile-relative offsets), exact for every L <= 32768.
+__device__ __forceinline__ uint32_t div_L(const Params& p, uint32_t d)
+{
+    return p.logL >= 0 ? (d >> p.logL) : (uint32_t)(((uint64_t)d * p.divL) >> 40);
+}
+
+// 4 bits (bit j = byte j of a equals byte j of b)
+__device__ __forceinline__ uint32_t eq_bytes4(uint32_t a, uint32_t b)
+{
+    return ((__vcmpeq4(a, b) & 0x08040201u) * 0x01010101u) >> 24;
+}
+
+// spread 4 bits to 4 bytes of 0/1
+__device__ __forceinline__ uint32_t bits_to_bytes4(uint32_t b)
+{
+    return ((b & 0xFu) * 0x00204081u) & 0x01010101u;
+}
+
+__device__ __forceinline__ uint32_t lanemask_lt()
+{
+    uint32_t m;
+    asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+    return m;
+}
+
+// Device-side accumulators at the start of the workspace (zeroed by sw_bind; parts re-zeroed per call).
+struct Acc {
+    unsigned long long n_active;       // bonds activated by the last sweep / step
+    unsigned long long n_clusters;     // roots counted by the last flatten pass
+    unsigned long long sat;            // observables
+    unsigned long long cnt[8];
+    unsigned long long cs_nclusters;   // cluster statistics
+    unsigned long long cs_max;
+    unsigned long long cs_sumsq;
+    unsigned long long hist[32];
+};
+constexpr int WOLFF_RING = 1024;       // per-step |C| slots between host flushes
+
+}  // namespace swb

@@ -1,0 +1,161 @@
+// misc_kernels.cuh -- support kernels: initialisation (S:8a a8), materialised bond activation (a1, sw_activate),
+// energy / magnetisation reduction (a6) and cluster statistics (a9).
+#pragma once
+#include "common.cuh"
+
+namespace swb {
+
+__device__ __forceinline__ uint32_t store_byte(int q, uint32_t k)
+{
+    return q == 2 ? (k ? 0xFFu : 0x01u) : k;             // Ising storage: k=0 -> +1, k=1 -> -1
+}
+
+// S:8c.8: cold: all k=0; random: k_i = (PHILOX(seed; i>>2, 0, 0, INIT)[i&3] * q) >> 32.  One thread per 4 sites.
+__global__ void __launch_bounds__(256)
+k_init(const Params p, uint32_t* __restrict__ spins_w, int mode)
+{
+    const int nw = p.N >> 2;
+    for (int i4 = blockIdx.x * blockDim.x + threadIdx.x; i4 < nw; i4 += gridDim.x * blockDim.x) {
+        uint32_t k0 = 0, k1 = 0, k2 = 0, k3 = 0;
+        if (mode == 1) {
+            uint32_t w0, w1, w2, w3;
+            philox4x32_10(p, (uint32_t)i4, 0u, 0u, DOM_INIT, w0, w1, w2, w3);
+            k0 = __umulhi(w0, (uint32_t)p.q); k1 = __umulhi(w1, (uint32_t)p.q);
+            k2 = __umulhi(w2, (uint32_t)p.q); k3 = __umulhi(w3, (uint32_t)p.q);
+        }
+        spins_w[i4] = store_byte(p.q, k0) | (store_byte(p.q, k1) << 8) | (store_byte(p.q, k2) << 16) |
+                      (store_byte(p.q, k3) << 24);
+    }
+}
+
+// Packed bonds of step t for the current spins (P:70 bond array; S:8c.3-4).  One thread per 4 sites = one byte.
+__global__ void __launch_bounds__(256)
+k_activate(const Params p, const uint32_t* __restrict__ spins_w, uint8_t* __restrict__ bonds)
+{
+    const int L = p.L, Lw = L >> 2, nw = p.N >> 2;
+    for (int i4 = blockIdx.x * blockDim.x + threadIdx.x; i4 < nw; i4 += gridDim.x * blockDim.x) {
+        const int yy = i4 / Lw, xw = i4 - yy * Lw;
+        const uint32_t w = spins_w[i4];
+        const uint32_t we = spins_w[yy * Lw + (xw + 1 == Lw ? 0 : xw + 1)];
+        const uint32_t wn = spins_w[(yy + 1 == L ? 0 : yy + 1) * Lw + xw];
+        const uint32_t eqe = eq_bytes4(w, __funnelshift_r(w, we, 8));
+        const uint32_t eqn = eq_bytes4(w, wn);
+        const uint32_t c0 = (uint32_t)i4 * 2u;           // (i>>1) of the first pair of this word
+        uint32_t a0, a1, a2, a3, b0, b1, b2, b3;
+        philox4x32_10(p, c0, p.t_lo, p.t_hi, DOM_BOND, a0, a1, a2, a3);
+        philox4x32_10(p, c0 + 1, p.t_lo, p.t_hi, DOM_BOND, b0, b1, b2, b3);
+        const uint32_t e0 = (eqe & 1u) && a0 < p.T, n0 = (eqn & 1u) && a1 < p.T;
+        const uint32_t e1 = (eqe & 2u) && a2 < p.T, n1 = (eqn & 2u) && a3 < p.T;
+        const uint32_t e2 = (eqe & 4u) && b0 < p.T, n2 = (eqn & 4u) && b1 < p.T;
+        const uint32_t e3 = (eqe & 8u) && b2 < p.T, n3 = (eqn & 8u) && b3 < p.T;
+        bonds[i4] = (uint8_t)(e0 | (n0 << 1) | (e1 << 2) | (n1 << 3) | (e2 << 4) | (n2 << 5) | (e3 << 6) | (n3 << 7));
+    }
+}
+
+__device__ __forceinline__ unsigned long long warp_sum_u64(unsigned long long v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// S:8a a6 (Eq. 1): satisfied bonds and per-state counts of the current spins, int64 accumulation:
+// registers -> warp shuffle -> one 64-bit atomic per warp and quantity.
+__global__ void __launch_bounds__(256)
+k_observables(const Params p, const uint32_t* __restrict__ spins_w, Acc* __restrict__ acc)
+{
+    const int L = p.L, Lw = L >> 2, nw = p.N >> 2;
+    unsigned long long sat = 0, cnt[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    for (int i4 = blockIdx.x * blockDim.x + threadIdx.x; i4 < nw; i4 += gridDim.x * blockDim.x) {
+        const int yy = i4 / Lw, xw = i4 - yy * Lw;
+        const uint32_t w = spins_w[i4];
+        const uint32_t we = spins_w[yy * Lw + (xw + 1 == Lw ? 0 : xw + 1)];
+        const uint32_t wn = spins_w[(yy + 1 == L ? 0 : yy + 1) * Lw + xw];
+        sat += __popc(eq_bytes4(w, __funnelshift_r(w, we, 8))) + __popc(eq_bytes4(w, wn));
+        if (p.q == 2) {
+            cnt[1] += __popc(w & 0x80808080u);           // bytes equal to -1
+        } else {
+#pragma unroll
+            for (int k = 1; k < 8; ++k)
+                if (k < p.q) cnt[k] += __popc(__vcmpeq4(w, 0x01010101u * k) & 0x01010101u);
+        }
+    }
+    sat = warp_sum_u64(sat);
+#pragma unroll
+    for (int k = 1; k < 8; ++k) cnt[k] = warp_sum_u64(cnt[k]);
+    if ((threadIdx.x & 31) == 0) {
+        if (sat) atomicAdd(&acc->sat, sat);
+#pragma unroll
+        for (int k = 1; k < 8; ++k) if (cnt[k]) atomicAdd(&acc->cnt[k], cnt[k]);
+    }
+}
+
+// S:8a a9: size[r] = number of sites with label r.  Equal labels in consecutive sites are merged in registers, then
+// across the warp with match_any, so that a giant cluster costs one atomic per warp instead of one per site.
+__global__ void __launch_bounds__(256)
+k_cluster_sizes(const Params p, const int* __restrict__ labels, int* __restrict__ size)
+{
+    const int nv = p.N >> 2;
+    for (int i4 = blockIdx.x * blockDim.x + threadIdx.x; i4 < ((nv + 31) & ~31); i4 += gridDim.x * blockDim.x) {
+        int lab[4] = {-1, -2, -3, -4};
+        int cnt[4] = {0, 0, 0, 0};
+        if (i4 < nv) {
+            const int4 v = reinterpret_cast<const int4*>(labels)[i4];
+            lab[0] = v.x; lab[1] = v.y; lab[2] = v.z; lab[3] = v.w;
+            cnt[0] = cnt[1] = cnt[2] = cnt[3] = 1;
+#pragma unroll
+            for (int j = 1; j < 4; ++j)
+                if (lab[j] == lab[j - 1]) { cnt[j] += cnt[j - 1]; cnt[j - 1] = 0; }
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int key = cnt[j] ? lab[j] : -1 - (int)(threadIdx.x & 31) - 32 * j;   // inactive: unique key
+            const uint32_t peers = __match_any_sync(0xffffffffu, key);
+            int tot = 0;
+            for (uint32_t m = peers; m; m &= m - 1) tot += __shfl_sync(peers, cnt[j], __ffs(m) - 1);
+            if (cnt[j] && (threadIdx.x & 31) == (uint32_t)(__ffs(peers) - 1)) atomicAdd(&size[key], tot);
+        }
+    }
+}
+
+// Statistics over the roots (labels[i] == i): count, maximum, sum of squares, log2-binned histogram.
+__global__ void __launch_bounds__(256)
+k_cluster_stats(const Params p, const int* __restrict__ labels, const int* __restrict__ size, Acc* __restrict__ acc)
+{
+    __shared__ unsigned long long s_hist[32];
+    __shared__ unsigned long long s_n, s_max, s_sq;
+    if (threadIdx.x < 32) s_hist[threadIdx.x] = 0;
+    if (threadIdx.x == 0) { s_n = 0; s_max = 0; s_sq = 0; }
+    __syncthreads();
+    unsigned long long n = 0, mx = 0, sq = 0;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < p.N; i += gridDim.x * blockDim.x) {
+        if (labels[i] == i) {
+            const unsigned long long s = (unsigned long long)(unsigned)size[i];
+            ++n;
+            mx = s > mx ? s : mx;
+            sq += s * s;
+            atomicAdd(&s_hist[31 - __clz((unsigned)s)], 1ull);
+        }
+    }
+    n = warp_sum_u64(n);
+    sq = warp_sum_u64(sq);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const unsigned long long other = __shfl_xor_sync(0xffffffffu, mx, o);
+        mx = other > mx ? other : mx;
+    }
+    if ((threadIdx.x & 31) == 0) {
+        atomicAdd(&s_n, n);
+        atomicAdd(&s_sq, sq);
+        atomicMax(&s_max, mx);
+    }
+    __syncthreads();
+    if (threadIdx.x < 32 && s_hist[threadIdx.x]) atomicAdd(&acc->hist[threadIdx.x], s_hist[threadIdx.x]);
+    if (threadIdx.x == 0) {
+        if (s_n) atomicAdd(&acc->cs_nclusters, s_n);
+        if (s_sq) atomicAdd(&acc->cs_sumsq, s_sq);
+        atomicMax(&acc->cs_max, s_max);
+    }
+}
+
+}  // namespace swb

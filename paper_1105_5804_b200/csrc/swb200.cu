@@ -1,0 +1,391 @@
+// swb200.cu -- the C-ABI of libswb200.so (include/swb200.h): host-side state, argument checks, kernel launches.
+// Every step of the path runs in the kernels of label_kernels.cuh / misc_kernels.cuh; there is no CPU fallback.
+#include "../../include/swb200.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "common.cuh"
+#include "label_kernels.cuh"
+#include "misc_kernels.cuh"
+
+using namespace swb;
+
+struct sw_handle {
+    int32_t  L, q;
+    int64_t  N;
+    double   beta;
+    uint64_t seed;
+    uint64_t t;                // step counter
+    uint32_t T;
+    Params   p;                // kernel parameters (t_lo/t_hi refreshed per launch)
+    // bound device buffers (caller-owned)
+    uint32_t* d_spins;
+    int32_t*  d_labels;
+    uint8_t*  d_bonds;
+    uint8_t*  d_work;
+    // carved from d_work
+    Acc*      d_acc;
+    unsigned long long* d_wolff;   // WOLFF_RING slots
+    uint8_t*  d_seam;              // seamE (ntx*L) followed by seamN (nty*L)
+    int32_t*  d_size;              // N int32
+    bool      bound;
+    bool      have_labels;         // a labelling has happened since bind
+    uint64_t  launches;
+    char      cuda_err[256];
+};
+
+namespace {
+
+constexpr size_t ALIGN = 256;
+inline size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
+
+struct WorkLayout { size_t acc, wolff, seam, size, total; };
+
+WorkLayout work_layout(int32_t L)
+{
+    const size_t N = (size_t)L * L;
+    const size_t ntx = (L + TW - 1) / TW, nty = (L + TH - 1) / TH;
+    WorkLayout w;
+    w.acc = 0;
+    w.wolff = align_up(sizeof(Acc));
+    w.seam = w.wolff + align_up(sizeof(unsigned long long) * WOLFF_RING);
+    w.size = w.seam + align_up((ntx + nty) * (size_t)L);
+    w.total = w.size + align_up(N * sizeof(int32_t));
+    return w;
+}
+
+bool valid_shape(int32_t L, int32_t q) { return L >= 4 && L <= 32768 && (L % 4) == 0 && q >= 2 && q <= 8; }
+
+int cuda_fail(sw_handle* h, cudaError_t e, const char* where)
+{
+    if (h) snprintf(h->cuda_err, sizeof(h->cuda_err), "%s: %s", where, cudaGetErrorString(e));
+    return SW_ECUDA;
+}
+
+#define SW_CUDA(h, call)                                                     \
+    do {                                                                     \
+        cudaError_t e__ = (call);                                            \
+        if (e__ != cudaSuccess) return cuda_fail((h), e__, #call);           \
+    } while (0)
+
+#define SW_LAUNCHED(h, name)                                                 \
+    do {                                                                     \
+        cudaError_t e__ = cudaGetLastError();                                \
+        if (e__ != cudaSuccess) return cuda_fail((h), e__, name);            \
+        ++(h)->launches;                                                     \
+    } while (0)
+
+uint32_t threshold_of(int32_t q, double beta)
+{
+    // S:8c.4 / reading 6: floor((1 - exp(-K beta)) 2^32) in IEEE double, K = 2 for q = 2 (Ising +-1), else 1
+    const double K = (q == 2) ? 2.0 : 1.0;
+    double v = std::floor((1.0 - std::exp(-K * beta)) * 4294967296.0);
+    if (v < 0.0) v = 0.0;
+    if (v > 4294967295.0) v = 4294967295.0;
+    return (uint32_t)v;
+}
+
+Params params_at(const sw_handle* h, uint64_t t)
+{
+    Params p = h->p;
+    p.T = h->T;
+    p.t_lo = (uint32_t)(t & 0xFFFFFFFFu);
+    p.t_hi = (uint32_t)(t >> 32);
+    return p;
+}
+
+inline int grid_for(int64_t n, int block) { return (int)((n + block - 1) / block); }
+inline int grid_capped(int64_t n, int block, int cap) { int g = grid_for(n, block); return g < cap ? (g < 1 ? 1 : g) : cap; }
+
+// labelling of the bond graph of step t (or of packed bonds): k_local -> k_seam -> k_seamfix
+template <bool FROM_BONDS>
+int launch_label_front(sw_handle* h, const Params& p, const uint8_t* bonds, int32_t* labels, cudaStream_t s)
+{
+    const dim3 grid(p.ntx, p.nty);
+    uint8_t* seamE = h->d_seam;
+    uint8_t* seamN = h->d_seam + (size_t)p.ntx * p.L;
+    k_local<FROM_BONDS><<<grid, NTHREADS, 0, s>>>(p, h->d_spins, bonds, labels, seamE, seamN, h->d_acc);
+    SW_LAUNCHED(h, "k_local");
+    const int nseam = (p.ntx + p.nty) * p.L;
+    k_seam<<<grid_for(nseam, 256), 256, 0, s>>>(p, h->d_seam, labels);
+    SW_LAUNCHED(h, "k_seam");
+    k_seamfix<<<grid_for(nseam, 256), 256, 0, s>>>(p, h->d_seam, labels);
+    SW_LAUNCHED(h, "k_seamfix");
+    return SW_OK;
+}
+
+int zero_sweep_counters(sw_handle* h, cudaStream_t s)
+{
+    // n_active and n_clusters are adjacent at the start of Acc
+    SW_CUDA(h, cudaMemsetAsync(h->d_acc, 0, 2 * sizeof(unsigned long long), s));
+    return SW_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* sw_strerror(int code)
+{
+    switch (code) {
+        case SW_OK: return "ok";
+        case SW_EINVAL: return "invalid argument";
+        case SW_ESTATE: return "handle not bound, or a needed buffer was bound as NULL";
+        case SW_ECUDA: return "CUDA error (see sw_last_cuda_error)";
+        case SW_ENOMEM: return "out of host memory";
+        default: return "unknown error code";
+    }
+}
+
+const char* sw_last_cuda_error(const sw_handle* h) { return h ? h->cuda_err : ""; }
+
+int sw_create(sw_handle** out, int32_t L, int32_t q, double beta, uint64_t seed)
+{
+    if (!out) return SW_EINVAL;
+    *out = nullptr;
+    if (!valid_shape(L, q) || !std::isfinite(beta) || beta < 0.0) return SW_EINVAL;
+    sw_handle* h = new (std::nothrow) sw_handle;
+    if (!h) return SW_ENOMEM;
+    memset(h, 0, sizeof(*h));
+    h->L = L; h->q = q; h->N = (int64_t)L * L; h->beta = beta; h->seed = seed; h->t = 0;
+    h->T = threshold_of(q, beta);
+    Params& p = h->p;
+    p.L = L; p.N = (int32_t)h->N; p.q = q;
+    p.logL = -1;
+    for (int k = 2; k <= 15; ++k) if ((1 << k) == L) p.logL = k;
+    p.ntx = (L + TW - 1) / TW; p.nty = (L + TH - 1) / TH;
+    p.divL = ((1ull << 40) + (uint64_t)L - 1) / (uint64_t)L;
+    const uint32_t s_lo = (uint32_t)(seed & 0xFFFFFFFFu), s_hi = (uint32_t)(seed >> 32);
+    for (int r = 0; r < 10; ++r) {
+        p.k0[r] = s_lo + (uint32_t)r * 0x9E3779B9u;
+        p.k1[r] = s_hi + (uint32_t)r * 0xBB67AE85u;
+    }
+    *out = h;
+    return SW_OK;
+}
+
+int sw_destroy(sw_handle* h)
+{
+    if (!h) return SW_EINVAL;
+    delete h;
+    return SW_OK;
+}
+
+size_t sw_workspace_bytes(int32_t L, int32_t q)
+{
+    if (!valid_shape(L, q)) return 0;
+    return work_layout(L).total;
+}
+
+int sw_bind(sw_handle* h, void* d_spins, int32_t* d_labels, uint8_t* d_bonds, void* d_work, size_t work_bytes,
+            void* stream)
+{
+    if (!h || !d_spins || !d_labels || !d_work) return SW_EINVAL;
+    if (((uintptr_t)d_spins | (uintptr_t)d_labels | (uintptr_t)d_bonds | (uintptr_t)d_work) & 15u) return SW_EINVAL;
+    const WorkLayout w = work_layout(h->L);
+    if (work_bytes < w.total) return SW_EINVAL;
+    h->d_spins = (uint32_t*)d_spins;
+    h->d_labels = d_labels;
+    h->d_bonds = d_bonds;
+    h->d_work = (uint8_t*)d_work;
+    h->d_acc = (Acc*)(h->d_work + w.acc);
+    h->d_wolff = (unsigned long long*)(h->d_work + w.wolff);
+    h->d_seam = h->d_work + w.seam;
+    h->d_size = (int32_t*)(h->d_work + w.size);
+    h->bound = false;
+    h->have_labels = false;
+    SW_CUDA(h, cudaMemsetAsync(h->d_work, 0, w.seam, (cudaStream_t)stream));
+    h->bound = true;
+    return SW_OK;
+}
+
+int sw_set_threshold(sw_handle* h, uint32_t T) { if (!h) return SW_EINVAL; h->T = T; return SW_OK; }
+int sw_get_threshold(const sw_handle* h, uint32_t* T) { if (!h || !T) return SW_EINVAL; *T = h->T; return SW_OK; }
+int sw_set_counter(sw_handle* h, uint64_t t) { if (!h) return SW_EINVAL; h->t = t; return SW_OK; }
+int sw_get_counter(const sw_handle* h, uint64_t* t) { if (!h || !t) return SW_EINVAL; *t = h->t; return SW_OK; }
+int sw_launch_count(const sw_handle* h, uint64_t* n) { if (!h || !n) return SW_EINVAL; *n = h->launches; return SW_OK; }
+
+int sw_init_spins(sw_handle* h, int mode, void* stream)
+{
+    if (!h || (mode != 0 && mode != 1)) return SW_EINVAL;
+    if (!h->bound) return SW_ESTATE;
+    const Params p = params_at(h, 0);
+    k_init<<<grid_capped(h->N / 4, 256, 148 * 16), 256, 0, (cudaStream_t)stream>>>(p, h->d_spins, mode);
+    SW_LAUNCHED(h, "k_init");
+    return SW_OK;
+}
+
+int sw_sweep(sw_handle* h, int64_t n, void* stream)
+{
+    if (!h || n < 0) return SW_EINVAL;
+    if (!h->bound) return SW_ESTATE;
+    cudaStream_t s = (cudaStream_t)stream;
+    for (int64_t k = 0; k < n; ++k) {
+        const Params p = params_at(h, h->t);
+        int rc = zero_sweep_counters(h, s);
+        if (rc) return rc;
+        rc = launch_label_front<false>(h, p, nullptr, h->d_labels, s);
+        if (rc) return rc;
+        k_final<MODE_SW><<<dim3(p.ntx, p.nty), NTHREADS, 0, s>>>(p, h->d_labels, h->d_spins, h->d_acc, nullptr);
+        SW_LAUNCHED(h, "k_final<SW>");
+        ++h->t;
+        h->have_labels = true;
+    }
+    return SW_OK;
+}
+
+int sw_activate(sw_handle* h, void* stream)
+{
+    if (!h) return SW_EINVAL;
+    if (!h->bound || !h->d_bonds) return SW_ESTATE;
+    const Params p = params_at(h, h->t);
+    k_activate<<<grid_capped(h->N / 4, 256, 148 * 16), 256, 0, (cudaStream_t)stream>>>(p, h->d_spins, h->d_bonds);
+    SW_LAUNCHED(h, "k_activate");
+    return SW_OK;
+}
+
+int sw_label(sw_handle* h, const uint8_t* d_bonds_in, int32_t* d_labels_out, void* stream)
+{
+    if (!h) return SW_EINVAL;
+    if (!h->bound) return SW_ESTATE;
+    const uint8_t* bonds = d_bonds_in ? d_bonds_in : h->d_bonds;
+    int32_t* labels = d_labels_out ? d_labels_out : h->d_labels;
+    if (!bonds) return SW_ESTATE;
+    if (((uintptr_t)bonds | (uintptr_t)labels) & 15u) return SW_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    const Params p = params_at(h, h->t);
+    int rc = zero_sweep_counters(h, s);
+    if (rc) return rc;
+    rc = launch_label_front<true>(h, p, bonds, labels, s);
+    if (rc) return rc;
+    k_final<MODE_LABEL><<<dim3(p.ntx, p.nty), NTHREADS, 0, s>>>(p, labels, nullptr, h->d_acc, nullptr);
+    SW_LAUNCHED(h, "k_final<LABEL>");
+    if (labels == h->d_labels) h->have_labels = true;
+    return SW_OK;
+}
+
+static int cluster_stats_device(sw_handle* h, const int32_t* labels, cudaStream_t s)
+{
+    const Params p = params_at(h, h->t);
+    SW_CUDA(h, cudaMemsetAsync(h->d_size, 0, (size_t)h->N * sizeof(int32_t), s));
+    SW_CUDA(h, cudaMemsetAsync(&h->d_acc->cs_nclusters, 0, sizeof(unsigned long long) * (3 + 32), s));
+    k_cluster_sizes<<<grid_capped(h->N / 4, 256, 148 * 16), 256, 0, s>>>(p, labels, h->d_size);
+    SW_LAUNCHED(h, "k_cluster_sizes");
+    k_cluster_stats<<<grid_capped(h->N, 256, 148 * 8), 256, 0, s>>>(p, labels, h->d_size, h->d_acc);
+    SW_LAUNCHED(h, "k_cluster_stats");
+    return SW_OK;
+}
+
+int sw_cluster_stats(sw_handle* h, const int32_t* d_labels_in, sw_cstats* h_out, void* stream)
+{
+    if (!h || !h_out) return SW_EINVAL;
+    if (!h->bound) return SW_ESTATE;
+    const int32_t* labels = d_labels_in ? d_labels_in : h->d_labels;
+    if ((uintptr_t)labels & 15u) return SW_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    int rc = cluster_stats_device(h, labels, s);
+    if (rc) return rc;
+    Acc a;
+    SW_CUDA(h, cudaMemcpyAsync(&a, h->d_acc, sizeof(Acc), cudaMemcpyDeviceToHost, s));
+    SW_CUDA(h, cudaStreamSynchronize(s));
+    h_out->n_clusters = (int64_t)a.cs_nclusters;
+    h_out->max_cluster = (int64_t)a.cs_max;
+    h_out->sum_sq_cluster = a.cs_sumsq;
+    for (int b = 0; b < 32; ++b) h_out->hist32[b] = (int64_t)a.hist[b];
+    return SW_OK;
+}
+
+int wolff_step(sw_handle* h, int64_t n, int64_t* h_sizes, void* stream)
+{
+    if (!h || n < 0) return SW_EINVAL;
+    if (h->q != 2) return SW_EINVAL;                     // DESIGN.md reading 8: the paper defines Wolff for Ising only
+    if (!h->bound) return SW_ESTATE;
+    cudaStream_t s = (cudaStream_t)stream;
+    int64_t done = 0;
+    while (done < n) {
+        const int64_t batch = (n - done) < WOLFF_RING ? (n - done) : WOLFF_RING;
+        SW_CUDA(h, cudaMemsetAsync(h->d_wolff, 0, sizeof(unsigned long long) * (size_t)batch, s));
+        for (int64_t k = 0; k < batch; ++k) {
+            const Params p = params_at(h, h->t);
+            int rc = zero_sweep_counters(h, s);
+            if (rc) return rc;
+            rc = launch_label_front<false>(h, p, nullptr, h->d_labels, s);
+            if (rc) return rc;
+            k_final<MODE_WOLFF><<<dim3(p.ntx, p.nty), NTHREADS, 0, s>>>(p, h->d_labels, h->d_spins, h->d_acc,
+                                                                         h->d_wolff + k);
+            SW_LAUNCHED(h, "k_final<WOLFF>");
+            ++h->t;
+            h->have_labels = true;
+        }
+        if (h_sizes) {
+            SW_CUDA(h, cudaMemcpyAsync(h_sizes + done, h->d_wolff, sizeof(int64_t) * (size_t)batch,
+                                       cudaMemcpyDeviceToHost, s));
+            SW_CUDA(h, cudaStreamSynchronize(s));
+        }
+        done += batch;
+    }
+    return SW_OK;
+}
+
+int sw_observables(sw_handle* h, sw_obs* h_out, void* stream)
+{
+    if (!h || !h_out) return SW_EINVAL;
+    if (!h->bound) return SW_ESTATE;
+    cudaStream_t s = (cudaStream_t)stream;
+    const Params p = params_at(h, h->t);
+    SW_CUDA(h, cudaMemsetAsync(&h->d_acc->sat, 0, sizeof(unsigned long long) * 9, s));
+    k_observables<<<grid_capped(h->N / 4, 256, 148 * 8), 256, 0, s>>>(p, h->d_spins, h->d_acc);
+    SW_LAUNCHED(h, "k_observables");
+    if (h->have_labels) {
+        int rc = cluster_stats_device(h, h->d_labels, s);
+        if (rc) return rc;
+    }
+    Acc a;
+    SW_CUDA(h, cudaMemcpyAsync(&a, h->d_acc, sizeof(Acc), cudaMemcpyDeviceToHost, s));
+    SW_CUDA(h, cudaStreamSynchronize(s));
+    memset(h_out, 0, sizeof(*h_out));
+    const int64_t N = h->N;
+    h_out->sat_bonds = (int64_t)a.sat;
+    int64_t rest = 0;
+    for (int k = 1; k < h->q; ++k) { h_out->state_count[k] = (int64_t)a.cnt[k]; rest += (int64_t)a.cnt[k]; }
+    h_out->state_count[0] = N - rest;
+    if (h->q == 2) {
+        h_out->energy = -(2 * h_out->sat_bonds - 2 * N);
+        h_out->magnetisation = h_out->state_count[0] - h_out->state_count[1];
+    } else {
+        int64_t mx = 0;
+        for (int k = 0; k < h->q; ++k) if (h_out->state_count[k] > mx) mx = h_out->state_count[k];
+        h_out->energy = -h_out->sat_bonds;
+        h_out->magnetisation = (int64_t)h->q * mx - N;
+    }
+    if (h->have_labels) {
+        h_out->n_clusters = (int64_t)a.n_clusters;
+        h_out->n_active_bonds = (int64_t)a.n_active;
+        h_out->max_cluster = (int64_t)a.cs_max;
+        h_out->sum_sq_cluster = a.cs_sumsq;
+    }
+    h_out->counter = h->t;
+    return SW_OK;
+}
+
+int sw_sweep_host(sw_handle* h, const void* h_spins_in, int64_t n, void* h_spins_out, int32_t* h_labels_out,
+                  sw_obs* h_obs, void* stream)
+{
+    if (!h || n < 0) return SW_EINVAL;
+    if (!h->bound) return SW_ESTATE;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (h_spins_in) SW_CUDA(h, cudaMemcpyAsync(h->d_spins, h_spins_in, (size_t)h->N, cudaMemcpyHostToDevice, s));
+    int rc = sw_sweep(h, n, stream);
+    if (rc) return rc;
+    if (h_spins_out) SW_CUDA(h, cudaMemcpyAsync(h_spins_out, h->d_spins, (size_t)h->N, cudaMemcpyDeviceToHost, s));
+    if (h_labels_out)
+        SW_CUDA(h, cudaMemcpyAsync(h_labels_out, h->d_labels, (size_t)h->N * sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+    if (h_obs) return sw_observables(h, h_obs, stream);
+    SW_CUDA(h, cudaStreamSynchronize(s));
+    return SW_OK;
+}
+
+}  // extern "C"
