@@ -1,0 +1,322 @@
+#!/usr/bin/env python
+"""bench.py -- headline measurement: ns per spin update of a full Swendsen-Wang sweep at L=16384, beta_c, q=2
+(BASELINE.json metric; config 3 at beta_c), on N GPUs of one node as N independent replicas ("replicas only",
+DESIGN.md: the path is specified for one GPU and has no exchange step).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--L 16384] [--beta BETA] [--impl ours|reference]
+
+One JSON line on stdout (rank 0).  A "step" is one pass of the whole hot path -- bond activation, tile-local
+labelling, seam merge, flatten + flip -- over one L x L lattice.  Inputs (the spin configuration) are resident in
+HBM for `value`; `e2e` goes through sw_sweep_host with pinned HOST buffers, copies inside the timed region.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+PAPER_NS_L16384 = 3.573          # Table I, Tesla M2070, q=2, beta_c, L=16384 (context only)
+BYTES_PER_SITE_SWEEP = 14.0      # SURVEY 8(d) model (iii) / DESIGN.md: 1 + 4 + 4 + 4 + 1
+BYTES_PER_SITE = {"k_local": 5.0, "k_seam": 0.0, "k_seamfix": 0.0, "k_final": 9.0}   # DESIGN.md per-kernel table
+PHASES = ["k_local", "k_seam", "k_seamfix", "k_final"]
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture
+# (profiles/r01_ncu_full.md), bytes; None until a capture exists for that kernel.
+NCU_TRAFFIC = {"k_local": None, "k_final": None}
+
+
+def beta_c_ising() -> float:
+    return 0.5 * math.log(1.0 + math.sqrt(2.0))
+
+
+def measured_peak_gbs():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s; MEASURED_PEAKS.json absent)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except ValueError:
+                continue
+            for name, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def aggregate_over_ranks(local_ms: float, local_units: float, dist=None):
+    """Whole-job time = max over ranks, whole-job units = sum over ranks (weak scaling, independent replicas).
+    `dist` is torch.distributed (initialised) or None for a single process.  Works on gloo (CPU) and nccl."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return local_ms, local_units
+    import torch
+    dev = torch.device("cuda", torch.cuda.current_device()) if dist.get_backend() == "nccl" else torch.device("cpu")
+    t = torch.tensor([local_ms], dtype=torch.float64, device=dev)
+    u = torch.tensor([local_units], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+# ------------------------------------------------------------------------------------------------ reference arm
+def reference_sample_L(L: int, steps: int, warmup: int, budget_s: float = 150.0, ns_per_site: float = 160.0) -> int:
+    """Largest power-of-two lattice <= L whose (steps+warmup) oracle sweeps fit the time budget."""
+    per_step = budget_s / max(1, steps + warmup)
+    sites = per_step / (ns_per_site * 1e-9)
+    Ls = 64
+    while Ls * 2 <= L and (Ls * 2) ** 2 <= sites:
+        Ls *= 2
+    return Ls
+
+
+def time_oracle(L: int, beta: float, seed: int, steps: int, warmup: int, spins=None):
+    """ns per spin update of the oracle as it stands, one host thread (it is serial, like the paper's CPU code P:322)."""
+    import oracle
+    T = oracle.threshold(2, beta)
+    s = oracle.init_spins(L, 2, seed, 1) if spins is None else spins
+    t = 0
+    for _ in range(warmup):
+        oracle.sweep(L, 2, T, seed, t, s); t += 1
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        oracle.sweep(L, 2, T, seed, t, s); t += 1
+    dt = time.perf_counter() - t0
+    return dt / steps / (L * L) * 1e9, dt / steps * 1e3
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    Ls = reference_sample_L(args.L, args.steps, args.warmup)
+    ns, ms = time_oracle(Ls, args.beta, 1, args.steps, args.warmup)
+    sample = ("one serial oracle sweep per step on an L=%d periodic lattice at the same beta from a random start "
+              "(%d of the workload's %d sites per step), 1 thread" % (Ls, Ls * Ls, args.L * args.L))
+    line = {
+        "impl": "reference", "metric": "ns_per_spin_update", "value": ns, "unit": "ns", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": False,
+        "scaling": "weak", "vs_baseline": None, "dtype": "i32", "data": "synthetic",
+        "config": {"workload": "2D Ising SW sweep, L=%d periodic, beta=%.10f, q=2" % (args.L, args.beta),
+                   "L": args.L, "q": 2, "beta": args.beta},
+        "cpu_baseline": {"value": ns, "unit": "ns", "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": ns, "unit": "ns", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------ our arm
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1105_5804_b200 import binding
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU path")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    device = "cuda:%d" % local_rank
+
+    L, beta, N = args.L, args.beta, args.L * args.L
+    lat = binding.Lattice(L, 2, beta, 1 + rank, device=device)        # one independent replica per rank
+    lat.init_spins(1)
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing ----------------------------------------------------------------------------
+    lat.sweep(args.warmup)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    l0 = lat.launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record(stream)
+    lat.sweep(args.steps)
+    ev1.record(stream)
+    barrier()
+    local_ms = ev0.elapsed_time(ev1)
+    launches = lat.launch_count() - l0
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms, total_units = aggregate_over_ranks(local_ms, float(N) * args.steps, dist if world > 1 else None)
+    ms_per_step = total_ms / args.steps
+    ns_per_spin = total_ms * 1e6 / total_units
+
+    # ---- per-kernel split (instrumented pass, same state, same stream) ---------------------------------------
+    prof_steps = min(args.steps, 64)
+    lat.profile_enable(True)
+    lat.sweep(prof_steps)
+    phase_ms, nprof = lat.profile_read()
+    lat.profile_enable(False)
+    per_kernel = {name: phase_ms[i] / max(1, nprof) for i, name in enumerate(PHASES)}
+    obs = lat.observables()
+
+    # ---- end to end through the host-buffer entry point ----------------------------------------------------
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    h_in = torch.empty(N, dtype=torch.int8).pin_memory()
+    h_out = torch.empty(N, dtype=torch.int8).pin_memory()
+    h_in.copy_(lat.spins.cpu())
+    lat.sweep_host(h_in, 1, h_out, None)                              # warm-up
+    barrier()
+    ev0.record(stream)
+    for _ in range(e2e_steps):
+        o = lat.sweep_host(h_in, 1, h_out, None)                      # H2D spins, 1 sweep, D2H spins + observables
+        h_in, h_out = h_out, h_in
+    ev1.record(stream)
+    barrier()
+    e2e_ms, e2e_units = aggregate_over_ranks(ev0.elapsed_time(ev1), float(N) * e2e_steps, dist if world > 1 else None)
+    e2e_ns = e2e_ms * 1e6 / e2e_units
+
+    if rank != 0:
+        lat.close()
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline of the dominant kernel ---------------------------------------------------------------------
+    peak, peak_src = measured_peak_gbs()
+    dom = max(("k_local", "k_final"), key=lambda k: per_kernel[k])
+    dom_bytes = BYTES_PER_SITE[dom] * N
+    achieved = dom_bytes / (per_kernel[dom] * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": NCU_TRAFFIC.get(dom), "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": dom_bytes, "kernel_ms": per_kernel[dom],
+                "kernel_ms_all": per_kernel,
+                "kernel_share_of_step": per_kernel[dom] / max(1e-12, sum(per_kernel.values())),
+                "sweep": {"algorithmic_bytes": BYTES_PER_SITE_SWEEP * N,
+                          "achieved": BYTES_PER_SITE_SWEEP * N / (ms_per_step * 1e-3) / 1e9,
+                          "frac_of_measured_peak": BYTES_PER_SITE_SWEEP * N / (ms_per_step * 1e-3) / 1e9 / peak,
+                          "frac_of_8TBps_nominal": BYTES_PER_SITE_SWEEP * N / (ms_per_step * 1e-3) / 1e9 / 8000.0,
+                          "frac_compulsory_6B_of_measured_peak": 6.0 * N / (ms_per_step * 1e-3) / 1e9 / peak}}
+
+    # ---- the oracle on this box's host cores, bounded sample ---------------------------------------------------
+    cpu = None
+    if not args.no_cpu_baseline:
+        Ls = min(L, 4096)
+        lat_s = binding.Lattice(Ls, 2, beta, 1, device=device)
+        lat_s.init_spins(1)
+        lat_s.sweep(60)                                               # equilibrate the sample on the GPU
+        s = lat_s.spins_host().copy()
+        lat_s.close()
+        import oracle
+        T = oracle.threshold(2, beta)
+        nsw = 4 if Ls >= 4096 else 8
+        t0 = time.perf_counter()
+        for k in range(nsw):
+            oracle.sweep(Ls, 2, T, 1, 60 + k, s)
+        dt = time.perf_counter() - t0
+        cpu = {"value": dt / nsw / (Ls * Ls) * 1e9, "unit": "ns", "cores": 1, "kind": "oracle",
+               "sample": "%d serial oracle sweeps of an L=%d lattice at the same beta, started from a state "
+                         "equilibrated by 60 GPU sweeps (%.1f s of CPU work; host has %d cores, the oracle uses 1)"
+                         % (nsw, Ls, dt, os.cpu_count() or 0)}
+
+    line = {
+        "metric": "ns_per_spin_update", "value": ns_per_spin, "unit": "ns", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "weak",
+        "vs_baseline": ns_per_spin / PAPER_NS_L16384 if (L == 16384 and abs(beta - beta_c_ising()) < 1e-9) else None,
+        "dtype": "i32", "data": "synthetic",
+        "config": {"workload": "BASELINE.json configs[2] at beta_c: 2D Ising (q=2) Swendsen-Wang, L=%d periodic, "
+                               "beta=%.10f, random +-1 start from seed, int8 spins / int32 labels" % (L, beta),
+                   "L": L, "q": 2, "beta": beta, "sites_per_step": N, "replicas": world,
+                   "l2_policy": "inputs larger than L2: spins %d MiB + labels %d MiB per step vs 126 MB L2"
+                                % (N >> 20, (4 * N) >> 20),
+                   "sweeps_per_s": 1e3 / ms_per_step * world},
+        "clocks": clocks,
+        "e2e": {"value": e2e_ns, "unit": "ns", "h2d_bytes_per_step": N, "d2h_bytes_per_step": N + 128,
+                "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps,
+                "what": "sw_sweep_host: pinned host spins -> device, one sweep, spins + sw_obs back to the host"},
+        "gpu_launches": launches,
+        "roofline": roofline,
+        "cpu_baseline": cpu,
+        "state": {"energy_per_site": obs["energy"] / N, "magnetisation_per_site": obs["magnetisation"] / N,
+                  "clusters_per_site": obs["n_clusters"] / N, "largest_cluster_fraction": obs["max_cluster"] / N,
+                  "counter": obs["counter"]},
+    }
+    print(json.dumps(line), flush=True)
+    lat.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main(argv=None):
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=50)
+    ap.add_argument("--L", type=int, default=16384)
+    ap.add_argument("--beta", type=float, default=beta_c_ising())
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args(argv)
+    if args.warmup < 3:
+        args.warmup = 3
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

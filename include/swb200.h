@@ -136,6 +136,16 @@ int sw_observables(sw_handle* h, sw_obs* h_out, void* stream);
 int sw_sweep_host(sw_handle* h, const void* h_spins_in, int64_t n, void* h_spins_out, int32_t* h_labels_out,
                   sw_obs* h_obs, void* stream);
 
+/* Per-kernel timing of sw_sweep / sw_label with CUDA events on the launching stream (for roofline reporting; off by
+ * default, and the un-instrumented path records no events).  While enabled, each sweep records SW_NPHASE+1
+ * events; at most 512 sweeps are kept between reads (further sweeps run untimed).  sw_profile_read synchronises
+ * the recorded events, ADDS the elapsed milliseconds of each phase to ms[] and the number of timed sweeps to
+ * *n_sweeps, and clears the record.  Phases: 0 = k_local (activation + tile-local labelling), 1 = k_seam
+ * (cross-tile union-find), 2 = k_seamfix (seam root compression), 3 = k_final (flatten + flip). */
+#define SW_NPHASE 4
+int sw_profile_enable(sw_handle* h, int on);
+int sw_profile_read(sw_handle* h, double ms[SW_NPHASE], uint64_t* n_sweeps);
+
 /* Number of kernels this handle has launched so far (for bench.py's gpu_launches). */
 int sw_launch_count(const sw_handle* h, uint64_t* n);
 

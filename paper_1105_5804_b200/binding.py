@@ -19,7 +19,7 @@ SYMBOLS = [
     "sw_create", "sw_destroy", "sw_workspace_bytes", "sw_bind", "sw_set_threshold", "sw_get_threshold",
     "sw_set_counter", "sw_get_counter", "sw_init_spins", "sw_sweep", "sw_activate", "sw_label",
     "sw_cluster_stats", "wolff_step", "sw_observables", "sw_sweep_host", "sw_launch_count", "sw_strerror",
-    "sw_last_cuda_error",
+    "sw_last_cuda_error", "sw_profile_enable", "sw_profile_read",
 ]
 
 
@@ -75,6 +75,8 @@ def lib():
     L.sw_observables.argtypes = [vp, C.POINTER(sw_obs), vp]
     L.sw_sweep_host.argtypes = [vp, vp, i64, vp, vp, C.POINTER(sw_obs), vp]
     L.sw_launch_count.argtypes = [vp, C.POINTER(u64)]
+    L.sw_profile_enable.argtypes = [vp, C.c_int]
+    L.sw_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(u64)]
     L.sw_strerror.argtypes = [C.c_int]
     L.sw_strerror.restype = C.c_char_p
     L.sw_last_cuda_error.argtypes = [vp]
@@ -195,6 +197,16 @@ class Lattice:
             h_labels_out.data_ptr() if h_labels_out is not None else None,
             C.byref(out) if want_obs else None, self._stream()))
         return out.as_dict() if want_obs else None
+
+    def profile_enable(self, on: bool):
+        self._check(self._lib.sw_profile_enable(self._h, 1 if on else 0))
+
+    def profile_read(self):
+        """-> (ms per phase summed over the timed sweeps [k_local, k_seam, k_seamfix, k_final], number of sweeps)"""
+        ms = (C.c_double * 4)(0.0, 0.0, 0.0, 0.0)
+        n = C.c_uint64(0)
+        self._check(self._lib.sw_profile_read(self._h, ms, C.byref(n)))
+        return list(ms), n.value
 
     def launch_count(self) -> int:
         v = C.c_uint64()

@@ -20,12 +20,27 @@ __device__ __forceinline__ int uf_find(Ptr parent, int x)
     return x;
 }
 
+// find with path halving: every second node on the path is re-pointed at its grandparent.  The plain store races
+// with other finds and with atomicMin hooks; it only ever writes an ancestor of x, so the forest stays valid.
+__device__ __forceinline__ int uf_find_halve(volatile int* parent, int x)
+{
+    int p = parent[x];
+    while (p != x) {
+        const int gp = parent[p];
+        if (gp == p) return p;
+        parent[x] = gp;
+        x = gp;
+        p = parent[x];
+    }
+    return x;
+}
+
 __device__ __forceinline__ void uf_unite_shared(int* parent, int a, int b)
 {
     volatile int* vp = parent;
     while (true) {
-        a = uf_find(vp, a);
-        b = uf_find(vp, b);
+        a = uf_find_halve(vp, a);
+        b = uf_find_halve(vp, b);
         if (a == b) return;
         if (a < b) { int t = a; a = b; b = t; }          // a > b: hook a under b
         const int old = atomicMin(&parent[a], b);
@@ -64,6 +79,7 @@ k_local(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __r
         int* __restrict__ labels, uint8_t* __restrict__ seamE, uint8_t* __restrict__ seamN, Acc* __restrict__ acc)
 {
     __shared__ __align__(16) int parent[TW * TH];
+    __shared__ uint32_t s_efirst[NWARPS][32];            // east bonds of every warp's first row (4 bits per lane)
     constexpr int R = ROWS_PER_WARP;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int L = p.L;
@@ -141,6 +157,8 @@ k_local(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __r
         }
     }
 
+    s_efirst[warp][lane] = ebits & 0xFu;
+
     // run starts: every site points to the first site of its horizontal run inside the tile (HA4-style run labelling)
 #pragma unroll
     for (int r = 0; r < R; ++r) {
@@ -167,18 +185,22 @@ k_local(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __r
     }
     __syncthreads();
 
-    // north bonds: unite the run of (x,y) with the run of (x,y+1)
-#pragma unroll
-    for (int r = 0; r < R; ++r) {
-        const int ly = ly0 + r;
-        const uint32_t n4 = (nbits >> (4 * r)) & 0xFu;
-        if (n4) {                                        // implies a valid site with its north neighbour in the tile
-            const int4 a = *reinterpret_cast<const int4*>(&parent[ly * TW + 4 * lane]);
-            const int4 b = *reinterpret_cast<const int4*>(&parent[(ly + 1) * TW + 4 * lane]);
-            if (n4 & 1u) uf_unite_shared(parent, a.x, b.x);
-            if ((n4 & 2u) && !((n4 & 1u) && a.y == a.x && b.y == b.x)) uf_unite_shared(parent, a.y, b.y);
-            if ((n4 & 4u) && !((n4 & 2u) && a.z == a.y && b.z == b.y)) uf_unite_shared(parent, a.z, b.z);
-            if ((n4 & 8u) && !((n4 & 4u) && a.w == a.z && b.w == b.z)) uf_unite_shared(parent, a.w, b.w);
+    // north bonds: unite (x,y) with (x,y+1).  A bond is skipped when the site to its west has a north bond too and
+    // both horizontal bonds between the two columns are active (it joins the same two runs).  The remaining bonds
+    // of the thread's 8 rows are one 32-bit work mask, so lanes stay busy as long as they have any union left.
+    {
+        const uint32_t e_next = (warp + 1 < NWARPS) ? s_efirst[warp + 1][lane] : 0u;
+        const uint32_t e_up = (ebits >> 4) | (e_next << 28);          // east bonds of the row above each row
+        const uint32_t X = nbits & ebits & e_up;
+        uint32_t Xprev = __shfl_up_sync(0xffffffffu, X, 1);
+        if (lane == 0) Xprev = 0;
+        const uint32_t redundant = ((X << 1) & 0xEEEEEEEEu) | ((Xprev >> 3) & 0x11111111u);
+        uint32_t U = nbits & ~redundant;
+        while (U) {
+            const int b = __ffs(U) - 1;
+            U &= U - 1;
+            const int idx = (ly0 + (b >> 2)) * TW + 4 * lane + (b & 3);
+            uf_unite_shared(parent, idx, idx + TW);
         }
     }
     __syncthreads();
@@ -190,13 +212,14 @@ k_local(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __r
         if (y < L && colv) {
             const int4 a = *reinterpret_cast<const int4*>(&parent[ly * TW + 4 * lane]);
             int4 g;
-            int root = uf_find((volatile int*)parent, a.x);
+            volatile int* vp = parent;
+            int root = uf_find_halve(vp, a.x);
             g.x = (y0 + root / TW) * L + x0 + (root % TW);
-            if (a.y != a.x) root = uf_find((volatile int*)parent, a.y);
+            if (a.y != a.x) root = uf_find_halve(vp, a.y);
             g.y = (y0 + root / TW) * L + x0 + (root % TW);
-            if (a.z != a.y) root = uf_find((volatile int*)parent, a.z);
+            if (a.z != a.y) root = uf_find_halve(vp, a.z);
             g.z = (y0 + root / TW) * L + x0 + (root % TW);
-            if (a.w != a.z) root = uf_find((volatile int*)parent, a.w);
+            if (a.w != a.z) root = uf_find_halve(vp, a.w);
             g.w = (y0 + root / TW) * L + x0 + (root % TW);
             *reinterpret_cast<int4*>(labels + (size_t)y * L + x) = g;
         }
@@ -284,16 +307,39 @@ __device__ __forceinline__ uint32_t flip_state(const Params& p, int root)
     return __umulhi(w0, (uint32_t)p.q);                  // uniform state in [0,q)  (S:8c.6)
 }
 
+// Shared memory of k_final (dynamic, opt-in above 48 KB): the tile's provisional labels, one state byte per site
+// (only written at "anchor" sites) and the compacted list of anchor sites.
+struct FinalSmem {
+    int      S[TW * TH];
+    uint16_t list[TW * TH];
+    uint8_t  st[TW * TH];
+    int      nlist;
+};
+
+// tile-local index of global site v, or -1 if v lies outside the (possibly ragged) tile
+__device__ __forceinline__ int tile_local(const Params& p, int v, int base, int tw_eff, int th_eff)
+{
+    if (v < base) return -1;
+    const uint32_t d = (uint32_t)(v - base);
+    const uint32_t dy = div_L(p, d), dx = d - dy * (uint32_t)p.L;
+    return (dx < (uint32_t)tw_eff && dy < (uint32_t)th_eff) ? (int)(dy * TW + dx) : -1;
+}
+
 // One CTA per tile: canonical labels (root of every site) + the new spins.
 //   MODE_SW    : s_i = state drawn for the root (assign, P:55 step 3)
 //   MODE_WOLFF : s_i = -s_i iff root(i) == root(seed site i0); adds |C| to *wolff_size
 //   MODE_LABEL : labels only
+// After k_seamfix, root(i) = labels[labels[i]], and the second hop stays inside the tile unless labels[i] already is
+// the root.  "Anchor" sites are those whose own label is the final root (roots themselves, and sites pointing out
+// of the tile); only they draw a Philox state (compacted, one draw per anchor), every other site copies the state
+// of the anchor it resolves to through shared memory.
 template <int MODE>
-__global__ void __launch_bounds__(NTHREADS)
+__global__ void __launch_bounds__(NTHREADS, 4)
 k_final(const Params p, int* __restrict__ labels, uint32_t* __restrict__ spins_w, Acc* __restrict__ acc,
         unsigned long long* __restrict__ wolff_size)
 {
-    __shared__ __align__(16) int S[TW * TH];
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    FinalSmem& sm = *reinterpret_cast<FinalSmem*>(smem_raw);
     constexpr int R = ROWS_PER_WARP;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int L = p.L;
@@ -311,14 +357,49 @@ k_final(const Params p, int* __restrict__ labels, uint32_t* __restrict__ spins_w
         const int i0 = (int)__umulhi(w0, (uint32_t)p.N);
         r0 = __ldcg(labels + __ldcg(labels + i0));       // 2-hop guarantee; stable under concurrent k_final writes
     }
+    if (MODE == MODE_SW && threadIdx.x == 0) sm.nlist = 0;
 
-    int4 v[R];
+    uint32_t anchor = 0;                                 // bit 4r+j: my site (row r, column j) is an anchor
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         const int ly = ly0 + r, y = y0 + ly;
         if (y < L && colv) {
-            v[r] = *reinterpret_cast<const int4*>(labels + (size_t)y * L + x);
-            *reinterpret_cast<int4*>(&S[ly * TW + 4 * lane]) = v[r];
+            const int4 v = *reinterpret_cast<const int4*>(labels + (size_t)y * L + x);
+            *reinterpret_cast<int4*>(&sm.S[ly * TW + 4 * lane]) = v;
+            if (MODE == MODE_SW) {
+                const int i = y * L + x;
+                const int vv[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+                    if (vv[j] == i + j || tile_local(p, vv[j], base, tw_eff, th_eff) < 0) anchor |= 1u << (4 * r + j);
+            }
+        }
+    }
+
+    if (MODE == MODE_SW) {
+        __syncthreads();                                 // nlist = 0 visible
+        // compact the anchors of the whole tile into sm.list (warp scan + one shared atomic per warp)
+        const int cnt = __popc(anchor);
+        int incl = cnt;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += t;
+        }
+        int wbase = 0;
+        if (lane == 31) wbase = atomicAdd(&sm.nlist, incl);
+        wbase = __shfl_sync(0xffffffffu, wbase, 31);
+        int pos = wbase + incl - cnt;
+        for (uint32_t m = anchor; m; m &= m - 1) {
+            const int b = __ffs(m) - 1;
+            sm.list[pos++] = (uint16_t)((ly0 + (b >> 2)) * TW + 4 * lane + (b & 3));
+        }
+        __syncthreads();
+        // one Philox draw per anchor, balanced over the CTA
+        const int n = sm.nlist;
+        for (int k = threadIdx.x; k < n; k += NTHREADS) {
+            const int l = sm.list[k];
+            sm.st[l] = (uint8_t)flip_state(p, sm.S[l]);
         }
     }
     __syncthreads();
@@ -328,7 +409,8 @@ k_final(const Params p, int* __restrict__ labels, uint32_t* __restrict__ spins_w
     for (int r = 0; r < R; ++r) {
         const int ly = ly0 + r, y = y0 + ly;
         if (y < L && colv) {
-            const int vv[4] = {v[r].x, v[r].y, v[r].z, v[r].w};
+            const int4 v = *reinterpret_cast<const int4*>(&sm.S[ly * TW + 4 * lane]);
+            const int vv[4] = {v.x, v.y, v.z, v.w};
             int ww[4];
             uint32_t st[4];
             uint32_t old = 0;
@@ -337,29 +419,28 @@ k_final(const Params p, int* __restrict__ labels, uint32_t* __restrict__ spins_w
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 if (j > 0 && vv[j] == vv[j - 1]) { ww[j] = ww[j - 1]; st[j] = st[j - 1]; }
-                else {
-                    // second hop: through shared memory if the provisional root lies in this tile
-                    const uint32_t d = (uint32_t)(vv[j] - base);
+                else if (MODE == MODE_SW) {
+                    int l = ly * TW + 4 * lane + j;      // my own slot if I am an anchor
                     int w = vv[j];
-                    if (vv[j] >= base) {
-                        const uint32_t dy = div_L(p, d), dx = d - dy * (uint32_t)L;
-                        if (dx < (uint32_t)tw_eff && dy < (uint32_t)th_eff) w = S[dy * TW + dx];
+                    if (!((anchor >> (4 * r + j)) & 1u)) {
+                        l = tile_local(p, vv[j], base, tw_eff, th_eff);   // >= 0: non-anchors point into the tile
+                        w = sm.S[l];
+                        const int lw = tile_local(p, w, base, tw_eff, th_eff);
+                        if (lw >= 0) l = lw;             // root inside the tile: its own slot; else the hooked local root's
                     }
                     ww[j] = w;
-                    if (MODE == MODE_SW) st[j] = flip_state(p, w);
-                    else st[j] = 0;
+                    st[j] = sm.st[l];
+                } else {
+                    const int l = tile_local(p, vv[j], base, tw_eff, th_eff);
+                    ww[j] = l >= 0 ? sm.S[l] : vv[j];
+                    st[j] = 0;
                 }
                 nroots += (ww[j] == i + j);
             }
             *reinterpret_cast<int4*>(labels + (size_t)y * L + x) = make_int4(ww[0], ww[1], ww[2], ww[3]);
             if (MODE == MODE_SW) {
-                uint32_t word;
-                if (p.q == 2) {                          // k=0 -> +1 (0x01), k=1 -> -1 (0xFF)
-                    word = (st[0] ? 0xFFu : 0x01u) | (st[1] ? 0xFF00u : 0x0100u) |
-                           (st[2] ? 0xFF0000u : 0x010000u) | (st[3] ? 0xFF000000u : 0x01000000u);
-                } else {
-                    word = st[0] | (st[1] << 8) | (st[2] << 16) | (st[3] << 24);
-                }
+                uint32_t word = st[0] | (st[1] << 8) | (st[2] << 16) | (st[3] << 24);
+                if (p.q == 2) word = 0x01010101u | (word * 0xFEu);   // k=0 -> +1 (0x01), k=1 -> -1 (0xFF)
                 spins_w[((size_t)y * L + x) >> 2] = word;
             } else if (MODE == MODE_WOLFF) {
                 uint32_t m = 0;                          // bytes to negate

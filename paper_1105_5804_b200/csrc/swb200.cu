@@ -35,6 +35,10 @@ struct sw_handle {
     bool      have_labels;         // a labelling has happened since bind
     uint64_t  launches;
     char      cuda_err[256];
+    // optional per-kernel timing (sw_profile_*)
+    bool         prof_on;
+    int          prof_n;                                  // sweeps recorded since the last read
+    cudaEvent_t* prof_ev;                                 // PROF_MAX * (SW_NPHASE + 1) events, created on enable
 };
 
 namespace {
@@ -97,6 +101,12 @@ Params params_at(const sw_handle* h, uint64_t t)
     return p;
 }
 
+constexpr int PROF_MAX = 512;
+inline void prof_mark(sw_handle* h, int phase, cudaStream_t s)
+{
+    if (h->prof_on && h->prof_n < PROF_MAX) cudaEventRecord(h->prof_ev[h->prof_n * (SW_NPHASE + 1) + phase], s);
+}
+
 inline int grid_for(int64_t n, int block) { return (int)((n + block - 1) / block); }
 inline int grid_capped(int64_t n, int block, int cap) { int g = grid_for(n, block); return g < cap ? (g < 1 ? 1 : g) : cap; }
 
@@ -107,13 +117,17 @@ int launch_label_front(sw_handle* h, const Params& p, const uint8_t* bonds, int3
     const dim3 grid(p.ntx, p.nty);
     uint8_t* seamE = h->d_seam;
     uint8_t* seamN = h->d_seam + (size_t)p.ntx * p.L;
+    prof_mark(h, 0, s);
     k_local<FROM_BONDS><<<grid, NTHREADS, 0, s>>>(p, h->d_spins, bonds, labels, seamE, seamN, h->d_acc);
     SW_LAUNCHED(h, "k_local");
+    prof_mark(h, 1, s);
     const int nseam = (p.ntx + p.nty) * p.L;
     k_seam<<<grid_for(nseam, 256), 256, 0, s>>>(p, h->d_seam, labels);
     SW_LAUNCHED(h, "k_seam");
+    prof_mark(h, 2, s);
     k_seamfix<<<grid_for(nseam, 256), 256, 0, s>>>(p, h->d_seam, labels);
     SW_LAUNCHED(h, "k_seamfix");
+    prof_mark(h, 3, s);
     return SW_OK;
 }
 
@@ -167,9 +181,44 @@ int sw_create(sw_handle** out, int32_t L, int32_t q, double beta, uint64_t seed)
     return SW_OK;
 }
 
+int sw_profile_enable(sw_handle* h, int on)
+{
+    if (!h) return SW_EINVAL;
+    if (on && !h->prof_ev) {
+        h->prof_ev = new (std::nothrow) cudaEvent_t[PROF_MAX * (SW_NPHASE + 1)];
+        if (!h->prof_ev) return SW_ENOMEM;
+        for (int i = 0; i < PROF_MAX * (SW_NPHASE + 1); ++i) SW_CUDA(h, cudaEventCreate(&h->prof_ev[i]));
+    }
+    h->prof_on = on != 0;
+    h->prof_n = 0;
+    return SW_OK;
+}
+
+int sw_profile_read(sw_handle* h, double ms[SW_NPHASE], uint64_t* n_sweeps)
+{
+    if (!h || !ms || !n_sweeps) return SW_EINVAL;
+    if (!h->prof_ev) return SW_ESTATE;
+    for (int k = 0; k < h->prof_n; ++k) {
+        cudaEvent_t* e = h->prof_ev + k * (SW_NPHASE + 1);
+        SW_CUDA(h, cudaEventSynchronize(e[SW_NPHASE]));
+        for (int ph = 0; ph < SW_NPHASE; ++ph) {
+            float t = 0.f;
+            SW_CUDA(h, cudaEventElapsedTime(&t, e[ph], e[ph + 1]));
+            ms[ph] += (double)t;
+        }
+    }
+    *n_sweeps += (uint64_t)h->prof_n;
+    h->prof_n = 0;
+    return SW_OK;
+}
+
 int sw_destroy(sw_handle* h)
 {
     if (!h) return SW_EINVAL;
+    if (h->prof_ev) {
+        for (int i = 0; i < PROF_MAX * (SW_NPHASE + 1); ++i) cudaEventDestroy(h->prof_ev[i]);
+        delete[] h->prof_ev;
+    }
     delete h;
     return SW_OK;
 }
@@ -197,6 +246,9 @@ int sw_bind(sw_handle* h, void* d_spins, int32_t* d_labels, uint8_t* d_bonds, vo
     h->d_size = (int32_t*)(h->d_work + w.size);
     h->bound = false;
     h->have_labels = false;
+    SW_CUDA(h, cudaFuncSetAttribute(k_final<MODE_SW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FinalSmem)));
+    SW_CUDA(h, cudaFuncSetAttribute(k_final<MODE_WOLFF>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FinalSmem)));
+    SW_CUDA(h, cudaFuncSetAttribute(k_final<MODE_LABEL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FinalSmem)));
     SW_CUDA(h, cudaMemsetAsync(h->d_work, 0, w.seam, (cudaStream_t)stream));
     h->bound = true;
     return SW_OK;
@@ -229,8 +281,10 @@ int sw_sweep(sw_handle* h, int64_t n, void* stream)
         if (rc) return rc;
         rc = launch_label_front<false>(h, p, nullptr, h->d_labels, s);
         if (rc) return rc;
-        k_final<MODE_SW><<<dim3(p.ntx, p.nty), NTHREADS, 0, s>>>(p, h->d_labels, h->d_spins, h->d_acc, nullptr);
+        k_final<MODE_SW><<<dim3(p.ntx, p.nty), NTHREADS, sizeof(FinalSmem), s>>>(p, h->d_labels, h->d_spins, h->d_acc, nullptr);
         SW_LAUNCHED(h, "k_final<SW>");
+        prof_mark(h, 4, s);
+        if (h->prof_on && h->prof_n < PROF_MAX) ++h->prof_n;
         ++h->t;
         h->have_labels = true;
     }
@@ -261,8 +315,10 @@ int sw_label(sw_handle* h, const uint8_t* d_bonds_in, int32_t* d_labels_out, voi
     if (rc) return rc;
     rc = launch_label_front<true>(h, p, bonds, labels, s);
     if (rc) return rc;
-    k_final<MODE_LABEL><<<dim3(p.ntx, p.nty), NTHREADS, 0, s>>>(p, labels, nullptr, h->d_acc, nullptr);
+    k_final<MODE_LABEL><<<dim3(p.ntx, p.nty), NTHREADS, sizeof(int) * TW * TH, s>>>(p, labels, nullptr, h->d_acc, nullptr);
     SW_LAUNCHED(h, "k_final<LABEL>");
+    prof_mark(h, 4, s);
+    if (h->prof_on && h->prof_n < PROF_MAX) ++h->prof_n;
     if (labels == h->d_labels) h->have_labels = true;
     return SW_OK;
 }
@@ -314,9 +370,11 @@ int wolff_step(sw_handle* h, int64_t n, int64_t* h_sizes, void* stream)
             if (rc) return rc;
             rc = launch_label_front<false>(h, p, nullptr, h->d_labels, s);
             if (rc) return rc;
-            k_final<MODE_WOLFF><<<dim3(p.ntx, p.nty), NTHREADS, 0, s>>>(p, h->d_labels, h->d_spins, h->d_acc,
+            k_final<MODE_WOLFF><<<dim3(p.ntx, p.nty), NTHREADS, sizeof(int) * TW * TH, s>>>(p, h->d_labels, h->d_spins, h->d_acc,
                                                                          h->d_wolff + k);
             SW_LAUNCHED(h, "k_final<WOLFF>");
+            prof_mark(h, 4, s);
+            if (h->prof_on && h->prof_n < PROF_MAX) ++h->prof_n;
             ++h->t;
             h->have_labels = true;
         }
