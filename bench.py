@@ -26,11 +26,11 @@ if ROOT not in sys.path:
 
 PAPER_NS_L16384 = 3.573          # Table I, Tesla M2070, q=2, beta_c, L=16384 (context only)
 BYTES_PER_SITE_SWEEP = 14.0      # SURVEY 8(d) model (iii) / DESIGN.md: 1 + 4 + 4 + 4 + 1
-BYTES_PER_SITE = {"k_local": 5.0, "k_seam": 0.0, "k_seamfix": 0.0, "k_final": 9.0}   # DESIGN.md per-kernel table
-PHASES = ["k_local", "k_seam", "k_seamfix", "k_final"]
+BYTES_PER_SITE = {"k_scan": 5.0, "k_seam": 0.0, "k_final": 9.0}   # DESIGN.md per-kernel table
+PHASES = ["k_scan", "k_seam", "k_final"]
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture
 # (profiles/r01_ncu_full.md), bytes; None until a capture exists for that kernel.
-NCU_TRAFFIC = {"k_local": None, "k_final": None}
+NCU_TRAFFIC = {"k_scan": None, "k_final": None}
 
 
 def beta_c_ising() -> float:
@@ -236,7 +236,7 @@ def run_ours(args):
 
     # ---- roofline of the dominant kernel ---------------------------------------------------------------------
     peak, peak_src = measured_peak_gbs()
-    dom = max(("k_local", "k_final"), key=lambda k: per_kernel[k])
+    dom = max(("k_scan", "k_final"), key=lambda k: per_kernel[k])
     dom_bytes = BYTES_PER_SITE[dom] * N
     achieved = dom_bytes / (per_kernel[dom] * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",

@@ -140,9 +140,9 @@ int sw_sweep_host(sw_handle* h, const void* h_spins_in, int64_t n, void* h_spins
  * default, and the un-instrumented path records no events).  While enabled, each sweep records SW_NPHASE+1
  * events; at most 512 sweeps are kept between reads (further sweeps run untimed).  sw_profile_read synchronises
  * the recorded events, ADDS the elapsed milliseconds of each phase to ms[] and the number of timed sweeps to
- * *n_sweeps, and clears the record.  Phases: 0 = k_local (activation + tile-local labelling), 1 = k_seam
- * (cross-tile union-find), 2 = k_seamfix (seam root compression), 3 = k_final (flatten + flip). */
-#define SW_NPHASE 4
+ * *n_sweeps, and clears the record.  Phases: 0 = k_scan (activation + strip-local labelling), 1 = k_seam
+ * (cross-strip union-find), 2 = k_final (flatten + flip). */
+#define SW_NPHASE 3
 int sw_profile_enable(sw_handle* h, int on);
 int sw_profile_read(sw_handle* h, double ms[SW_NPHASE], uint64_t* n_sweeps);
 

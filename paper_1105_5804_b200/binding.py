@@ -13,6 +13,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libswb200.so")
 
 SW_OK, SW_EINVAL, SW_ESTATE, SW_ECUDA, SW_ENOMEM = 0, -1, -2, -3, -4
+NPHASE = 3                                                # SW_NPHASE of include/swb200.h
 
 # every symbol include/swb200.h declares (tests check that the library exports all of them)
 SYMBOLS = [
@@ -202,8 +203,8 @@ class Lattice:
         self._check(self._lib.sw_profile_enable(self._h, 1 if on else 0))
 
     def profile_read(self):
-        """-> (ms per phase summed over the timed sweeps [k_local, k_seam, k_seamfix, k_final], number of sweeps)"""
-        ms = (C.c_double * 4)(0.0, 0.0, 0.0, 0.0)
+        """-> (ms per phase summed over the timed sweeps [k_scan, k_seam, k_final], number of sweeps)"""
+        ms = (C.c_double * NPHASE)(*([0.0] * NPHASE))
         n = C.c_uint64(0)
         self._check(self._lib.sw_profile_read(self._h, ms, C.byref(n)))
         return list(ms), n.value

@@ -6,14 +6,19 @@
 
 namespace swb {
 
-// Tile of the one-level decomposition ("tiles of B_x x B_y spins", P:84 B_x >> B_y for coalescing).
-// One CTA of 256 threads labels a TW x TH tile held in shared memory: lane -> 4 consecutive columns (one 32-bit
-// word of int8 spins, one 128-bit vector of int32 labels), warp -> TH/8 consecutive rows.
-constexpr int TW = 128;
-constexpr int TH = 64;
-constexpr int NTHREADS = 256;
-constexpr int NWARPS = NTHREADS / 32;
-constexpr int ROWS_PER_WARP = TH / NWARPS;
+// Strip of the one-level decomposition ("tiles of B_x x B_y spins", P:84 B_x >> B_y for coalescing).
+// k_scan: one WARP labels a TW x TH strip, lane -> 4 consecutive columns (one 32-bit word of int8 spins, one 128-bit
+// vector of int32 labels), rows in sequence.  k_final: one CTA of FIN_THREADS threads per strip.
+constexpr int TW_LOG = 7, TH_LOG = 5;
+constexpr int TW = 1 << TW_LOG;
+constexpr int TH = 1 << TH_LOG;
+constexpr int SCAN_WARPS = 4;                            // strips per k_scan CTA (horizontally adjacent)
+constexpr int SCAN_THREADS = 32 * SCAN_WARPS;
+constexpr int FIN_THREADS = 256;
+constexpr int FIN_WARPS = FIN_THREADS / 32;
+static_assert(TW == 128, "lane -> 4 columns, 32 lanes");
+static_assert(TW * TH <= 65536, "strip-local indices are kept in uint16");
+static_assert(TH % FIN_WARPS == 0 && 4 * (TH / FIN_WARPS) <= 32, "k_final keeps one bit per site of a thread in a 32-bit mask");
 
 enum : uint32_t { DOM_INIT = 0, DOM_BOND = 1, DOM_FLIP = 2, DOM_WSEED = 3 };
 
@@ -26,7 +31,6 @@ struct Params {
     int32_t  ntx, nty;   // number of tile columns / rows
     uint32_t T;          // bond threshold floor(p 2^32)
     uint32_t t_lo, t_hi; // step counter
-    uint64_t divL;       // ceil(2^40 / L): d / L == (d * divL) >> 40 for d < 2^24
     uint32_t k0[10];     // Philox round keys: k0[r] = seed_lo + r * 0x9E3779B9
     uint32_t k1[10];     //                    k1[r] = seed_hi + r * 0xBB67AE85
 };
@@ -46,10 +50,10 @@ __device__ __forceinline__ void philox4x32_10(const Params& p, uint32_t c0, uint
     w0 = c0; w1 = c1; w2 = c2; w3 = c3;
 }
 
-// d / L for 0 <= d < 2^24 (tile-relative offsets), exact for every L <= 32768.
+// d / L (seam ids); a shift when L is a power of two.
 __device__ __forceinline__ uint32_t div_L(const Params& p, uint32_t d)
 {
-    return p.logL >= 0 ? (d >> p.logL) : (uint32_t)(((uint64_t)d * p.divL) >> 40);
+    return p.logL >= 0 ? (d >> p.logL) : d / (uint32_t)p.L;
 }
 
 // 4 bits (bit j = byte j of a equals byte j of b)

@@ -1,300 +1,351 @@
 // label_kernels.cuh -- the Swendsen-Wang hot path (S:8a rows a1-a5, a7):
-//   k_local   : bond activation (P:53 step 1, Eq. 7) fused with tile-local labelling in shared memory
-//   k_seam    : cross-tile consolidation as ONE concurrent union-find pass over the seam bonds
-//   k_seamfix : path compression of the seam roots so that every provisional label is at most 2 hops from its root
-//   k_final   : flatten to canonical labels + cluster flip (P:55 step 3) / Wolff flip / label only
+//   k_scan  : bond activation (P:53 step 1, Eq. 7) fused with strip-local labelling: one warp scans a
+//             TW x TH strip row by row, the labels of the previous row stay in registers, a run adopts the label of
+//             its first contact with the row above, and a (rare) union in a small shared-memory forest happens only
+//             when two different trees meet
+//   k_seam  : cross-strip consolidation as ONE concurrent union-find pass over the seam bonds
+//   k_final : flatten to canonical labels + cluster flip (P:55 step 3) / Wolff flip / label only
 // Design notes and the differences from the paper's kernels (self-labelling, hierarchical sewing) are in DESIGN.md.
+//
+// Provisional label array `prov` (the caller's int32 labels buffer) between k_scan and k_final:
+//   entry < 0  : REF | l  -- reference to the site with strip-local index l = ly * TW + lx of the SAME strip, l smaller
+//                than the site's own local index (a forest inside the strip)
+//   entry >= 0 : global site index g <= own index; g == own index: the site is the root of its tree.  Only
+//                strip-local roots carry entries >= 0; k_seam hooks them to roots of other strips (always to a smaller
+//                global index), so the root of every tree is the minimum site index of its cluster.
 #pragma once
 #include "common.cuh"
 
 namespace swb {
 
-// ------------------------------------------------------------------------------------------------ union-find
-// Lock-free union by minimum index on a parent array (shared or global memory).  Invariant: parent[x] <= x, and
-// parent[x] only ever changes to a smaller index of the same (growing) set, so a stale read is still an ancestor.
-template <typename Ptr>
-__device__ __forceinline__ int uf_find(Ptr parent, int x)
-{
-    int p = parent[x];
-    while (p != x) { x = p; p = parent[x]; }
-    return x;
-}
+constexpr int REF = (int)0x80000000;
+constexpr int LMASK = TW * TH - 1;
+constexpr int NONE = 0x7FFFFFFF;                         // "no contact" (any value >= 0 works)
+constexpr unsigned FULLM = 0xffffffffu;
 
-// find with path halving: every second node on the path is re-pointed at its grandparent.  The plain store races
-// with other finds and with atomicMin hooks; it only ever writes an ancestor of x, so the forest stays valid.
-__device__ __forceinline__ int uf_find_halve(volatile int* parent, int x)
+__device__ __forceinline__ int strip_gidx(int base, int L, int l) { return base + (l >> TW_LOG) * L + (l & (TW - 1)); }
+
+// ------------------------------------------------------------------------------------------------ k_scan
+// find with path halving in the strip's node table (uint16 parent per strip-local site index; only node entries are
+// ever written or read).  Plain loads/stores: the table is private to one warp, see the 3-phase protocol below.
+__device__ __forceinline__ int tbl_find(volatile uint16_t* tbl, int x)
 {
-    int p = parent[x];
+    int p = tbl[x];
     while (p != x) {
-        const int gp = parent[p];
+        const int gp = tbl[p];
         if (gp == p) return p;
-        parent[x] = gp;
+        tbl[x] = (uint16_t)gp;
         x = gp;
-        p = parent[x];
+        p = tbl[x];
     }
     return x;
 }
 
-__device__ __forceinline__ void uf_unite_shared(int* parent, int a, int b)
-{
-    volatile int* vp = parent;
-    while (true) {
-        a = uf_find_halve(vp, a);
-        b = uf_find_halve(vp, b);
-        if (a == b) return;
-        if (a < b) { int t = a; a = b; b = t; }          // a > b: hook a under b
-        const int old = atomicMin(&parent[a], b);
-        if (old == a) return;                            // a was a root and now points to b
-        a = old;                                         // a had been hooked meanwhile: parent[a] = min(old,b); join old and b
-    }
-}
-
-struct LdCg {                                            // global loads that bypass the (incoherent) L1
-    const int* p;
-    __device__ __forceinline__ int operator[](int i) const { return __ldcg(p + i); }
-};
-
-__device__ __forceinline__ void uf_unite_global(int* parent, int a, int b)
-{
-    LdCg vp{parent};
-    while (true) {
-        a = uf_find(vp, a);
-        b = uf_find(vp, b);
-        if (a == b) return;
-        if (a < b) { int t = a; a = b; b = t; }
-        const int old = atomicMin(&parent[a], b);
-        if (old == a) return;
-        a = old;
-    }
-}
-
-// ------------------------------------------------------------------------------------------------ k_local
-// One CTA per TW x TH tile.  FROM_BONDS=false: read spins, draw bonds (a1).  FROM_BONDS=true: read packed bonds
-// (sw_label).  Writes provisional labels (global index of the tile-local root = minimum index inside the tile),
-// the bonds that cross the tile's east / north edge into seamE / seamN (one byte per seam site), and adds the
-// number of active bonds to acc->n_active.
+// One warp per TW x TH strip, lane -> 4 consecutive columns, rows in sequence.  FROM_BONDS=false: read spins, draw
+// bonds (a1).  FROM_BONDS=true: read packed bonds (sw_label).  Writes the forest described above, the bonds that
+// cross the strip's east / north edge into seamE / seamN (one byte per seam site), and adds the number of active
+// bonds to acc->n_active.
+//
+// Row step.  A "node" is a horizontal run (inside the strip) that has no active north bond from the row above; it is
+// named by its first site.  Every other run adopts the name carried by its leftmost contact with the row above, so
+// all sites written are either nodes or references to nodes.  Only when a run has further contacts whose names
+// differ from the adopted one, the two names are united in the node table (hooking the larger index under the
+// smaller).  The strip-local root is therefore the minimum site index of the strip-local component.
 template <bool FROM_BONDS>
-__global__ void __launch_bounds__(NTHREADS)
-k_local(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __restrict__ bonds_in,
-        int* __restrict__ labels, uint8_t* __restrict__ seamE, uint8_t* __restrict__ seamN, Acc* __restrict__ acc)
+__global__ void __launch_bounds__(SCAN_THREADS)
+k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __restrict__ bonds_in, int* prov,
+       uint8_t* __restrict__ seamE, uint8_t* __restrict__ seamN, Acc* __restrict__ acc)
 {
-    __shared__ __align__(16) int parent[TW * TH];
-    __shared__ uint32_t s_efirst[NWARPS][32];            // east bonds of every warp's first row (4 bits per lane)
-    constexpr int R = ROWS_PER_WARP;
+    __shared__ uint16_t s_tbl[SCAN_WARPS][TW * TH];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int L = p.L;
-    const int x0 = blockIdx.x * TW, y0 = blockIdx.y * TH;
+    const int tx = blockIdx.x * SCAN_WARPS + warp, ty = blockIdx.y;
+    if (tx >= p.ntx) return;                             // no block-wide barrier in this kernel
+    volatile uint16_t* tbl = s_tbl[warp];
+    const int L = p.L, Lw = L >> 2;
+    const int x0 = tx * TW, y0 = ty * TH;
     const int tw_eff = min(TW, L - x0), th_eff = min(TH, L - y0);
     const int x = x0 + 4 * lane;
     const bool colv = 4 * lane < tw_eff;
-    const int last_lane = (tw_eff >> 2) - 1;             // lane that owns the tile's last column
-    const int ly0 = warp * R;
+    const int last_lane = (tw_eff >> 2) - 1;             // lane that owns the strip's last column
+    const bool is_last = lane == last_lane;
+    const int base = y0 * L + x0;
+    const int xw = x >> 2;
+    const int xew = ((x + 4 == L) ? 0 : x + 4) >> 2;     // east halo word of the last lane (periodic)
+    const unsigned lt = lanemask_lt(), me = 1u << lane, le = lt | me, gt = ~le;
 
-    uint32_t ebits = 0, nbits = 0;                       // 4 bits per row r at bit 4r
+    // spin words of rows y, y+1, y+2 (w*) and the east halo words of the last lane (h*); row index L wraps to 0
+    uint32_t w0 = 0, w1 = 0, w2 = 0, h0 = 0, h1 = 0, h2 = 0;
+    if (!FROM_BONDS) {
+        const int yend = y0 + th_eff;                    // north neighbour row of the strip's last row
+        if (colv) {
+            w0 = spins_w[(size_t)y0 * Lw + xw];
+            if (is_last) h0 = spins_w[(size_t)y0 * Lw + xew];
+            const int ya = y0 + 1, yb = y0 + 2;
+            if (ya <= yend) { const int yy = ya == L ? 0 : ya; w1 = spins_w[(size_t)yy * Lw + xw]; if (is_last) h1 = spins_w[(size_t)yy * Lw + xew]; }
+            if (yb <= yend) { const int yy = yb == L ? 0 : yb; w2 = spins_w[(size_t)yy * Lw + xw]; if (is_last) h2 = spins_w[(size_t)yy * Lw + xew]; }
+        }
+    }
+
+    int Lp0 = NONE, Lp1 = NONE, Lp2 = NONE, Lp3 = NONE;  // names carried by the previous row's sites
+    uint32_t np = 0;                                     // active north bonds from the previous row into this row
     int nact = 0;
 
-    if (!FROM_BONDS) {
-        const int Lw = L >> 2;                           // words per row
-        // my word in rows ly0 .. ly0+R (the last one is only the north neighbour of row R-1)
-        uint32_t w[R + 1];
-#pragma unroll
-        for (int r = 0; r <= R; ++r) {
-            const int y = y0 + ly0 + r;                  // y == L: periodic wrap, north neighbour of the last row
-            w[r] = (colv && y <= L) ? spins_w[(size_t)(y == L ? 0 : y) * Lw + (x >> 2)] : 0u;
-        }
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const int y = y0 + ly0 + r;
-            const bool rowv = y < L;                     // warp-uniform
-            uint32_t wnext = __shfl_down_sync(0xffffffffu, w[r], 1);
-            if (rowv && colv && lane == last_lane) {     // east halo: first word of the next tile (periodic)
-                const int xe = (x + 4 == L) ? 0 : x + 4;
-                wnext = spins_w[(size_t)y * Lw + (xe >> 2)];
+    for (int ly = 0; ly < th_eff; ++ly) {
+        const int y = y0 + ly;
+        uint32_t e4 = 0, n4 = 0;
+        if (!FROM_BONDS) {
+            uint32_t w3 = 0, h3 = 0;                     // prefetch row y+3
+            {
+                const int yc = y + 3;
+                if (colv && yc <= y0 + th_eff) {
+                    const int yy = yc == L ? 0 : yc;
+                    w3 = spins_w[(size_t)yy * Lw + xw];
+                    if (is_last) h3 = spins_w[(size_t)yy * Lw + xew];
+                }
             }
-            if (rowv && colv) {
-                const uint32_t east = __funnelshift_r(w[r], wnext, 8);
-                const uint32_t eqe = eq_bytes4(w[r], east);
-                const uint32_t eqn = eq_bytes4(w[r], w[r + 1]);
+            uint32_t wnext = __shfl_down_sync(FULLM, w0, 1);
+            if (is_last) wnext = h0;
+            if (colv) {
+                const uint32_t east = __funnelshift_r(w0, wnext, 8);
+                const uint32_t eqe = eq_bytes4(w0, east);
+                const uint32_t eqn = eq_bytes4(w0, w1);
                 const uint32_t c0 = (uint32_t)(y * L + x) >> 1;
                 uint32_t a0, a1, a2, a3, b0, b1, b2, b3;
                 philox4x32_10(p, c0, p.t_lo, p.t_hi, DOM_BOND, a0, a1, a2, a3);
                 philox4x32_10(p, c0 + 1, p.t_lo, p.t_hi, DOM_BOND, b0, b1, b2, b3);
                 const uint32_t de = (a0 < p.T) | ((a2 < p.T) << 1) | ((b0 < p.T) << 2) | ((b2 < p.T) << 3);
                 const uint32_t dn = (a1 < p.T) | ((a3 < p.T) << 1) | ((b1 < p.T) << 2) | ((b3 < p.T) << 3);
-                const uint32_t e4 = eqe & de, n4 = eqn & dn;
+                e4 = eqe & de;
+                n4 = eqn & dn;
                 nact += __popc(e4) + __popc(n4);
-                ebits |= e4 << (4 * r);
-                nbits |= n4 << (4 * r);
             }
+            w0 = w1; w1 = w2; w2 = w3; h0 = h1; h1 = h2; h2 = h3;
+        } else if (colv) {
+            const uint32_t b = bonds_in[((size_t)y * L + x) >> 2];
+            e4 = (b & 1) | ((b >> 1) & 2) | ((b >> 2) & 4) | ((b >> 3) & 8);
+            n4 = ((b >> 1) & 1) | ((b >> 2) & 2) | ((b >> 3) & 4) | ((b >> 4) & 8);
         }
-    } else {
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const int y = y0 + ly0 + r;
-            if (y < L && colv) {
-                const uint32_t b = bonds_in[((size_t)y * L + x) >> 2];
-                const uint32_t e4 = (b & 1) | ((b >> 1) & 2) | ((b >> 2) & 4) | ((b >> 3) & 8);
-                const uint32_t n4 = ((b >> 1) & 1) | ((b >> 2) & 2) | ((b >> 3) & 4) | ((b >> 4) & 8);
-                ebits |= e4 << (4 * r);
-                nbits |= n4 << (4 * r);
-            }
-        }
-    }
 
-    // bonds crossing the tile edge go to the seam arrays and are removed from the local masks
-#pragma unroll
-    for (int r = 0; r < R; ++r) {
-        const int ly = ly0 + r, y = y0 + ly;
-        if (y < L && colv) {
-            if (lane == last_lane) {
-                seamE[(size_t)blockIdx.x * L + y] = (uint8_t)((ebits >> (4 * r + 3)) & 1u);
-                ebits &= ~(8u << (4 * r));
+        // bonds that leave the strip go to the seam arrays and are dropped here
+        if (colv) {
+            if (is_last) {
+                seamE[(size_t)tx * L + y] = (uint8_t)(e4 >> 3);
+                e4 &= 7u;
             }
             if (ly == th_eff - 1) {
-                *reinterpret_cast<uint32_t*>(seamN + (size_t)blockIdx.y * L + x) = bits_to_bytes4(nbits >> (4 * r));
-                nbits &= ~(0xFu << (4 * r));
+                *reinterpret_cast<uint32_t*>(seamN + (size_t)ty * L + x) = bits_to_bytes4(n4);
+                n4 = 0;
             }
         }
-    }
 
-    s_efirst[warp][lane] = ebits & 0xFu;
+        // ---- names of this row's sites ----------------------------------------------------------------------
+        const bool E0 = e4 & 1u, E1 = e4 & 2u, E2 = e4 & 4u, E3 = e4 & 8u;
+        const bool full = (e4 & 7u) == 7u;
+        const bool EL = (__shfl_up_sync(FULLM, e4, 1) & 8u) && lane;
+        const int ref0 = REF | (ly * TW + 4 * lane);
+        // leftmost contact of every intra-lane segment: forward pass, then spread back from the segment end
+        const int c0 = (np & 1u) ? Lp0 : NONE, c1 = (np & 2u) ? Lp1 : NONE;
+        const int c2 = (np & 4u) ? Lp2 : NONE, c3 = (np & 8u) ? Lp3 : NONE;
+        const int f1 = (E0 && c0 < 0) ? c0 : c1;
+        const int f2 = (E1 && f1 < 0) ? f1 : c2;
+        const int f3 = (E2 && f2 < 0) ? f2 : c3;
+        const int g2 = E2 ? f3 : f2;
+        const int g1 = E1 ? g2 : f1;
+        const int g0 = E0 ? g1 : c0;
+        const int s1 = E0 ? 0 : 1, s2 = E1 ? s1 : 2, s3 = E2 ? s2 : 3;      // first site of each site's segment
+        const int pubP = g0;                                                // my prefix segment: contact or NONE
+        const int pubS = f3 < 0 ? f3 : ref0 + s3;                           // my suffix segment: contact or new node
 
-    // run starts: every site points to the first site of its horizontal run inside the tile (HA4-style run labelling)
-#pragma unroll
-    for (int r = 0; r < R; ++r) {
-        const int ly = ly0 + r;
-        const bool rowv = y0 + ly < L;                   // warp-uniform
-        const uint32_t e4 = (ebits >> (4 * r)) & 0xFu;
-        const uint32_t nf = __ballot_sync(0xffffffffu, e4 != 0xFu);
-        const uint32_t hz = ~e4 & 0xFu;                  // broken east bonds inside my group
-        const int brk = 4 * lane + (32 - __clz(hz));     // first site after my last broken bond (valid if hz != 0)
-        const uint32_t cand = nf & lanemask_lt();
-        const int src = cand ? 31 - __clz(cand) : 0;
-        int sin = __shfl_sync(0xffffffffu, brk, src);    // start of the run that enters my group from the west
-        if (!cand) sin = 0;
-        if (rowv && colv) {
-            int4 s;
-            const int base = ly * TW;
-            uint32_t z;
-            s.x = base + sin;
-            z = hz & 1u; s.y = base + (z ? 4 * lane + (32 - __clz(z)) : sin);
-            z = hz & 3u; s.z = base + (z ? 4 * lane + (32 - __clz(z)) : sin);
-            z = hz & 7u; s.w = base + (z ? 4 * lane + (32 - __clz(z)) : sin);
-            *reinterpret_cast<int4*>(&parent[base + 4 * lane]) = s;
+        // runs that cross lane boundaries: lanes a..b, a's suffix segment, full lanes, b's prefix segment
+        const unsigned LINK = __ballot_sync(FULLM, E3);
+        const unsigned FULLB = __ballot_sync(FULLM, full);
+        const unsigned CS = __ballot_sync(FULLM, f3 < 0);
+        const unsigned CP = __ballot_sync(FULLM, g0 < 0);
+        const unsigned nPTL = ~(FULLB & (LINK << 1));                       // lanes where a run cannot pass to the left
+        const unsigned nPTR = ~(FULLB & LINK);                              // ... to the right
+        const int a_le = 31 - __clz(nPTL & le);                             // bit 0 of nPTL is always set
+        const int a_lt = 31 - __clz(nPTL & lt);                             // -1 on lane 0 (unused there: EL = 0)
+        const int bS = E3 ? __ffs(nPTR & gt) - 1 : lane;                    // bit 31 of nPTR is always set
+        const unsigned MS = (CS & ((1u << bS) - 1u) & (FULLM << a_le)) | (CP & (1u << bS));
+        const int srcS = MS ? __ffs(MS) - 1 : a_le;
+        const unsigned MP = (CS & lt & (FULLM << (a_lt & 31))) | (CP & me);
+        const int srcP = MP ? __ffs(MP) - 1 : a_lt;
+        const int vS1 = __shfl_sync(FULLM, pubS, srcS & 31);
+        const int vP1 = __shfl_sync(FULLM, pubP, bS);
+        const int vS2 = __shfl_sync(FULLM, pubS, srcP & 31);
+        const int RS = (srcS == bS) ? vP1 : vS1;                            // name of the run my suffix segment is in
+        const int RP = (srcP == lane) ? g0 : vS2;                           // ... my prefix segment (if not full)
+        const bool useS = E3 || (full && EL), useP = EL && !full;
+
+        int l0 = g0 < 0 ? g0 : ref0;
+        int l1 = g1 < 0 ? g1 : ref0 + s1;
+        int l2 = g2 < 0 ? g2 : ref0 + s2;
+        int l3 = f3 < 0 ? f3 : ref0 + s3;
+        if (useP) { l0 = RP; if (s1 == 0) l1 = RP; if (s2 == 0) l2 = RP; }
+        if (useS) { l3 = RS; if (s2 == s3) l2 = RS; if (s1 == s3) l1 = RS; if (s3 == 0) l0 = RS; }
+
+        // new nodes of this row: root entries in the table (the global entry is written with the row below)
+        const bool new0 = l0 == ref0, new1 = l1 == ref0 + 1, new2 = l2 == ref0 + 2, new3 = l3 == ref0 + 3;
+        {
+            const int lb = ly * TW + 4 * lane;
+            if (new0) tbl[lb] = (uint16_t)lb;
+            if (new1) tbl[lb + 1] = (uint16_t)(lb + 1);
+            if (new2) tbl[lb + 2] = (uint16_t)(lb + 2);
+            if (new3) tbl[lb + 3] = (uint16_t)(lb + 3);
         }
-    }
-    __syncthreads();
 
-    // north bonds: unite (x,y) with (x,y+1).  A bond is skipped when the site to its west has a north bond too and
-    // both horizontal bonds between the two columns are active (it joins the same two runs).  The remaining bonds
-    // of the thread's 8 rows are one 32-bit work mask, so lanes stay busy as long as they have any union left.
-    {
-        const uint32_t e_next = (warp + 1 < NWARPS) ? s_efirst[warp + 1][lane] : 0u;
-        const uint32_t e_up = (ebits >> 4) | (e_next << 28);          // east bonds of the row above each row
-        const uint32_t X = nbits & ebits & e_up;
-        uint32_t Xprev = __shfl_up_sync(0xffffffffu, X, 1);
-        if (lane == 0) Xprev = 0;
-        const uint32_t redundant = ((X << 1) & 0xEEEEEEEEu) | ((Xprev >> 3) & 0x11111111u);
-        uint32_t U = nbits & ~redundant;
-        while (U) {
-            const int b = __ffs(U) - 1;
-            U &= U - 1;
-            const int idx = (ly0 + (b >> 2)) * TW + 4 * lane + (b & 3);
-            uf_unite_shared(parent, idx, idx + TW);
+        // contacts whose carried name differs from the adopted one: unite the two trees.
+        // 3-phase protocol, no atomics (the table belongs to this warp): (1) all lanes find roots -- nobody hooks, so
+        // a root stays a root; (2) hook larger under smaller with a plain store -- lanes hooking the same root
+        // collide, one store wins; (3) re-read: losers retry.  Every successful hook is written through to `prov`.
+        unsigned um = ((np & 1u) && Lp0 != l0 ? 1u : 0u) | ((np & 2u) && Lp1 != l1 ? 2u : 0u) |
+                      ((np & 4u) && Lp2 != l2 ? 4u : 0u) | ((np & 8u) && Lp3 != l3 ? 8u : 0u);
+        if (__any_sync(FULLM, um != 0)) {
+            int ua = 0, ub = 0;
+            bool have = false;
+            while (true) {
+                if (!have && um) {
+                    const int c = __ffs(um) - 1;
+                    um &= um - 1;
+                    ua = (c == 0 ? Lp0 : c == 1 ? Lp1 : c == 2 ? Lp2 : Lp3) & LMASK;
+                    ub = (c == 0 ? l0 : c == 1 ? l1 : c == 2 ? l2 : l3) & LMASK;
+                    have = true;
+                }
+                if (!__any_sync(FULLM, have)) break;
+                __syncwarp();
+                if (have) {
+                    ua = tbl_find(tbl, ua);
+                    ub = tbl_find(tbl, ub);
+                    if (ua == ub) have = false;
+                    else if (ua < ub) { const int t = ua; ua = ub; ub = t; }
+                }
+                __syncwarp();
+                if (have) tbl[ua] = (uint16_t)ub;
+                __syncwarp();
+                if (have && tbl[ua] == ub) {
+                    prov[strip_gidx(base, L, ua)] = REF | ub;
+                    have = false;
+                }
+            }
         }
-    }
-    __syncthreads();
 
-    // resolve every site to its tile-local root and write the root's global index
-#pragma unroll
-    for (int r = 0; r < R; ++r) {
-        const int ly = ly0 + r, y = y0 + ly;
-        if (y < L && colv) {
-            const int4 a = *reinterpret_cast<const int4*>(&parent[ly * TW + 4 * lane]);
-            int4 g;
-            volatile int* vp = parent;
-            int root = uf_find_halve(vp, a.x);
-            g.x = (y0 + root / TW) * L + x0 + (root % TW);
-            if (a.y != a.x) root = uf_find_halve(vp, a.y);
-            g.y = (y0 + root / TW) * L + x0 + (root % TW);
-            if (a.z != a.y) root = uf_find_halve(vp, a.z);
-            g.z = (y0 + root / TW) * L + x0 + (root % TW);
-            if (a.w != a.z) root = uf_find_halve(vp, a.w);
-            g.w = (y0 + root / TW) * L + x0 + (root % TW);
-            *reinterpret_cast<int4*>(labels + (size_t)y * L + x) = g;
+        if (colv) {
+            const int gi = y * L + x;
+            int4 o;
+            o.x = new0 ? gi : l0;
+            o.y = new1 ? gi + 1 : l1;
+            o.z = new2 ? gi + 2 : l2;
+            o.w = new3 ? gi + 3 : l3;
+            *reinterpret_cast<int4*>(prov + (size_t)gi) = o;
         }
+        Lp0 = l0; Lp1 = l1; Lp2 = l2; Lp3 = l3;
+        np = n4;
     }
 
     if (!FROM_BONDS) {
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) nact += __shfl_xor_sync(0xffffffffu, nact, o);
+        for (int o = 16; o > 0; o >>= 1) nact += __shfl_xor_sync(FULLM, nact, o);
         if (lane == 0 && nact) atomicAdd(&acc->n_active, (unsigned long long)nact);
     }
 }
 
 // ------------------------------------------------------------------------------------------------ seams
-// Seam site id -> the two end sites of its crossing bond.  ids [0, ntx*L): east seams (tile column tc, row y);
-// ids [ntx*L, (ntx+nty)*L): north seams (tile row tr, column x).
-__device__ __forceinline__ void seam_sites(const Params& p, int id, int& a, int& b)
+// Seam site id -> the two end sites of its crossing bond and the origins of the strips they lie in.
+// ids [0, ntx*L): east seams (strip column tc, row y); ids [ntx*L, (ntx+nty)*L): north seams (strip row tr, column x).
+__device__ __forceinline__ void seam_sites(const Params& p, int id, int& a, int& b, int& base_a, int& base_b)
 {
     const int L = p.L;
     const int nE = p.ntx * L;
     if (id < nE) {
         const int tc = div_L(p, (uint32_t)id), y = id - tc * L;
         const int xs = min((tc + 1) * TW, L) - 1;
+        const int xb = xs + 1 == L ? 0 : xs + 1;
+        const int yb0 = (y >> TH_LOG) << TH_LOG;
         a = y * L + xs;
-        b = y * L + (xs + 1 == L ? 0 : xs + 1);
+        b = y * L + xb;
+        base_a = yb0 * L + tc * TW;
+        base_b = yb0 * L + xb;
     } else {
         const int k = id - nE;
         const int tr = div_L(p, (uint32_t)k), x = k - tr * L;
         const int ys = min((tr + 1) * TH, L) - 1;
+        const int yb = ys + 1 == L ? 0 : ys + 1;
+        const int xb0 = (x >> TW_LOG) << TW_LOG;
         a = ys * L + x;
-        b = (ys + 1 == L ? 0 : ys + 1) * L + x;
+        b = yb * L + x;
+        base_a = tr * TH * L + xb0;
+        base_b = yb * L + xb0;
     }
 }
 
-// One thread per seam site: if its crossing bond is active, unite the provisional roots of its two ends.
+// strip-local root (global index) of `site`: follow the strip-local references
+__device__ __forceinline__ int strip_root(const int* prov, int L, int site, int base)
+{
+    int cur = site;
+    int v = __ldcg(prov + cur);
+    while (v < 0) {
+        cur = strip_gidx(base, L, v & LMASK);
+        v = __ldcg(prov + cur);
+    }
+    return cur;
+}
+
+// Lock-free union by minimum index over the strip-local roots (entries >= 0).  Invariant: entry[x] <= x, and an entry
+// only ever changes to a smaller index of the same (growing) set, so a stale read is still an ancestor.  Path halving
+// writes an ancestor with a plain store; it can race with the atomicMin of a retrying hook, which then still unites
+// the displaced parent.
+__device__ __forceinline__ int gfind_halve(int* prov, int x)
+{
+    int pp = __ldcg(prov + x);
+    while (pp != x) {
+        const int gp = __ldcg(prov + pp);
+        if (gp == pp) return pp;
+        prov[x] = gp;
+        x = gp;
+        pp = __ldcg(prov + x);
+    }
+    return x;
+}
+
+__device__ __forceinline__ int gfind(const int* prov, int x)
+{
+    int pp = __ldcg(prov + x);
+    while (pp != x) { x = pp; pp = __ldcg(prov + x); }
+    return x;
+}
+
+__device__ __forceinline__ void gunite(int* prov, int a, int b)
+{
+    while (true) {
+        a = gfind_halve(prov, a);
+        b = gfind_halve(prov, b);
+        if (a == b) return;
+        if (a < b) { const int t = a; a = b; b = t; }    // a > b: hook a under b
+        const int old = atomicMin(prov + a, b);
+        if (old == a) return;                            // a was a root and now points to b
+        a = old;                                         // a had been hooked meanwhile: entry = min(old,b); join old and b
+    }
+}
+
+// One thread per seam site: if its crossing bond is active, unite the strip-local roots of its two ends.
 // `seam` is seamE followed by seamN (contiguous).
 __global__ void __launch_bounds__(256)
-k_seam(const Params p, const uint8_t* __restrict__ seam, int* __restrict__ labels)
+k_seam(const Params p, const uint8_t* __restrict__ seam, int* prov)
 {
     const int nseam = (p.ntx + p.nty) * p.L;
     const int id = blockIdx.x * blockDim.x + threadIdx.x;
     const bool on = id < nseam && seam[id];
     int ra = -1, rb = -1;
     if (on) {
-        int a, b;
-        seam_sites(p, id, a, b);
-        ra = __ldcg(labels + a);
-        rb = __ldcg(labels + b);
+        int a, b, base_a, base_b;
+        seam_sites(p, id, a, b, base_a, base_b);
+        ra = strip_root(prov, p.L, a, base_a);
+        rb = strip_root(prov, p.L, b, base_b);
     }
-    // the previous seam site joins the same two provisional clusters: skip (its thread does the union)
-    const int pa = __shfl_up_sync(0xffffffffu, ra, 1), pb = __shfl_up_sync(0xffffffffu, rb, 1);
+    // the previous seam site joins the same two strip-local clusters: skip (its thread does the union)
+    const int pa = __shfl_up_sync(FULLM, ra, 1), pb = __shfl_up_sync(FULLM, rb, 1);
     const bool dup = (threadIdx.x & 31) != 0 && pa == ra && pb == rb;
-    if (on && !dup) uf_unite_global(labels, ra, rb);
-}
-
-// After k_seam: for both ends of every active seam bond, point the site and its provisional root straight at the
-// final root.  Every provisional root that was hooked has such a site in its tile-local cluster, so afterwards
-// root(i) = labels[labels[i]] for every site i (2-hop guarantee used by k_final).
-__global__ void __launch_bounds__(256)
-k_seamfix(const Params p, const uint8_t* __restrict__ seam, int* __restrict__ labels)
-{
-    const int nseam = (p.ntx + p.nty) * p.L;
-    const int id = blockIdx.x * blockDim.x + threadIdx.x;
-    if (id >= nseam || !seam[id]) return;
-    int s[2];
-    seam_sites(p, id, s[0], s[1]);
-    LdCg vp{labels};
-#pragma unroll
-    for (int e = 0; e < 2; ++e) {
-        const int x1 = vp[s[e]];
-        const int g = uf_find(vp, x1);
-        if (x1 != g) {                                   // every writer stores the same final root: benign
-            labels[x1] = g;
-            labels[s[e]] = g;
-        }
-    }
+    if (on && !dup) gunite(prov, ra, rb);
 }
 
 // ------------------------------------------------------------------------------------------------ k_final
@@ -307,109 +358,110 @@ __device__ __forceinline__ uint32_t flip_state(const Params& p, int root)
     return __umulhi(w0, (uint32_t)p.q);                  // uniform state in [0,q)  (S:8c.6)
 }
 
-// Shared memory of k_final (dynamic, opt-in above 48 KB): the tile's provisional labels, one state byte per site
-// (only written at "anchor" sites) and the compacted list of anchor sites.
+// Shared memory of k_final: the strip's forest, one state byte per strip-local root, the compacted list of roots.
 struct FinalSmem {
     int      S[TW * TH];
     uint16_t list[TW * TH];
     uint8_t  st[TW * TH];
     int      nlist;
+    int      r0;
 };
 
-// tile-local index of global site v, or -1 if v lies outside the (possibly ragged) tile
-__device__ __forceinline__ int tile_local(const Params& p, int v, int base, int tw_eff, int th_eff)
-{
-    if (v < base) return -1;
-    const uint32_t d = (uint32_t)(v - base);
-    const uint32_t dy = div_L(p, d), dx = d - dy * (uint32_t)p.L;
-    return (dx < (uint32_t)tw_eff && dy < (uint32_t)th_eff) ? (int)(dy * TW + dx) : -1;
-}
-
-// One CTA per tile: canonical labels (root of every site) + the new spins.
+// One CTA per strip: canonical labels (root of every site) + the new spins.
 //   MODE_SW    : s_i = state drawn for the root (assign, P:55 step 3)
 //   MODE_WOLFF : s_i = -s_i iff root(i) == root(seed site i0); adds |C| to *wolff_size
 //   MODE_LABEL : labels only
-// After k_seamfix, root(i) = labels[labels[i]], and the second hop stays inside the tile unless labels[i] already is
-// the root.  "Anchor" sites are those whose own label is the final root (roots themselves, and sites pointing out
-// of the tile); only they draw a Philox state (compacted, one draw per anchor), every other site copies the state
-// of the anchor it resolves to through shared memory.
+// Strip-local roots (entries >= 0) are compacted into a list; each is resolved to the root of its global tree (a
+// chase over entries >= 0 of other strips, which concurrently running CTAs may already have overwritten with final
+// labels -- those are roots of the same tree, so the chase still ends at the right root) and draws one Philox state.
+// Every other site follows its strip-local references through shared memory.
 template <int MODE>
-__global__ void __launch_bounds__(NTHREADS, 4)
-k_final(const Params p, int* __restrict__ labels, uint32_t* __restrict__ spins_w, Acc* __restrict__ acc,
+__global__ void __launch_bounds__(FIN_THREADS)
+k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __restrict__ acc,
         unsigned long long* __restrict__ wolff_size)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    FinalSmem& sm = *reinterpret_cast<FinalSmem*>(smem_raw);
-    constexpr int R = ROWS_PER_WARP;
+    __shared__ __align__(16) FinalSmem sm;
+    constexpr int R = TH / FIN_WARPS;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int L = p.L;
     const int x0 = blockIdx.x * TW, y0 = blockIdx.y * TH;
-    const int tw_eff = min(TW, L - x0), th_eff = min(TH, L - y0);
+    const int tw_eff = min(TW, L - x0);
     const int x = x0 + 4 * lane;
     const bool colv = 4 * lane < tw_eff;
     const int ly0 = warp * R;
     const int base = y0 * L + x0;
 
-    int r0 = -1;
-    if (MODE == MODE_WOLFF) {
-        uint32_t w0, w1, w2, w3;
-        philox4x32_10(p, 0u, p.t_lo, p.t_hi, DOM_WSEED, w0, w1, w2, w3);
-        const int i0 = (int)__umulhi(w0, (uint32_t)p.N);
-        r0 = __ldcg(labels + __ldcg(labels + i0));       // 2-hop guarantee; stable under concurrent k_final writes
+    if (threadIdx.x == 0) {
+        sm.nlist = 0;
+        if (MODE == MODE_WOLFF) {
+            uint32_t w0, w1, w2, w3;
+            philox4x32_10(p, 0u, p.t_lo, p.t_hi, DOM_WSEED, w0, w1, w2, w3);
+            const int i0 = (int)__umulhi(w0, (uint32_t)p.N);
+            const int iy = i0 / L, ix = i0 - iy * L;
+            const int b0 = ((iy >> TH_LOG) << TH_LOG) * L + ((ix >> TW_LOG) << TW_LOG);
+            sm.r0 = gfind(labels, strip_root(labels, L, i0, b0));
+        }
     }
-    if (MODE == MODE_SW && threadIdx.x == 0) sm.nlist = 0;
 
-    uint32_t anchor = 0;                                 // bit 4r+j: my site (row r, column j) is an anchor
+    uint32_t rootm = 0;                                  // bit 4r+j: my site (row r, column j) is a strip-local root
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         const int ly = ly0 + r, y = y0 + ly;
         if (y < L && colv) {
             const int4 v = *reinterpret_cast<const int4*>(labels + (size_t)y * L + x);
             *reinterpret_cast<int4*>(&sm.S[ly * TW + 4 * lane]) = v;
-            if (MODE == MODE_SW) {
-                const int i = y * L + x;
-                const int vv[4] = {v.x, v.y, v.z, v.w};
-#pragma unroll
-                for (int j = 0; j < 4; ++j)
-                    if (vv[j] == i + j || tile_local(p, vv[j], base, tw_eff, th_eff) < 0) anchor |= 1u << (4 * r + j);
-            }
+            const int i = y * L + x;
+            if (MODE == MODE_SW)
+                rootm |= ((v.x >= 0) | ((v.y >= 0) << 1) | ((v.z >= 0) << 2) | ((v.w >= 0) << 3)) << (4 * r);
+            else                                         // only hooked roots need work
+                rootm |= ((v.x >= 0 && v.x != i) | ((v.y >= 0 && v.y != i + 1) << 1) | ((v.z >= 0 && v.z != i + 2) << 2) |
+                          ((v.w >= 0 && v.w != i + 3) << 3)) << (4 * r);
         }
     }
+    __syncthreads();                                     // nlist = 0, r0 and S visible
 
-    if (MODE == MODE_SW) {
-        __syncthreads();                                 // nlist = 0 visible
-        // compact the anchors of the whole tile into sm.list (warp scan + one shared atomic per warp)
-        const int cnt = __popc(anchor);
+    // compact the roots of the whole strip into sm.list (warp scan + one shared atomic per warp)
+    {
+        const int cnt = __popc(rootm);
         int incl = cnt;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
-            const int t = __shfl_up_sync(0xffffffffu, incl, o);
+            const int t = __shfl_up_sync(FULLM, incl, o);
             if (lane >= o) incl += t;
         }
         int wbase = 0;
-        if (lane == 31) wbase = atomicAdd(&sm.nlist, incl);
-        wbase = __shfl_sync(0xffffffffu, wbase, 31);
+        if (lane == 31 && incl) wbase = atomicAdd(&sm.nlist, incl);
+        wbase = __shfl_sync(FULLM, wbase, 31);
         int pos = wbase + incl - cnt;
-        for (uint32_t m = anchor; m; m &= m - 1) {
+        for (uint32_t m = rootm; m; m &= m - 1) {
             const int b = __ffs(m) - 1;
             sm.list[pos++] = (uint16_t)((ly0 + (b >> 2)) * TW + 4 * lane + (b & 3));
         }
-        __syncthreads();
-        // one Philox draw per anchor, balanced over the CTA
+    }
+    __syncthreads();
+    // one global resolve + one Philox draw per strip-local root, balanced over the CTA
+    {
         const int n = sm.nlist;
-        for (int k = threadIdx.x; k < n; k += NTHREADS) {
+        for (int k = threadIdx.x; k < n; k += FIN_THREADS) {
             const int l = sm.list[k];
-            sm.st[l] = (uint8_t)flip_state(p, sm.S[l]);
+            int v = sm.S[l];
+            if (v != strip_gidx(base, L, l)) {           // hooked by k_seam: find the root of the global tree
+                v = gfind(labels, v);
+                sm.S[l] = v;
+            }
+            if (MODE == MODE_SW) sm.st[l] = (uint8_t)flip_state(p, v);
         }
     }
     __syncthreads();
 
+    const int r0 = MODE == MODE_WOLFF ? sm.r0 : -1;
     int nroots = 0, nflip = 0;
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         const int ly = ly0 + r, y = y0 + ly;
         if (y < L && colv) {
-            const int4 v = *reinterpret_cast<const int4*>(&sm.S[ly * TW + 4 * lane]);
+            const int lb = ly * TW + 4 * lane;
+            const int4 v = *reinterpret_cast<const int4*>(&sm.S[lb]);
             const int vv[4] = {v.x, v.y, v.z, v.w};
             int ww[4];
             uint32_t st[4];
@@ -418,22 +470,12 @@ k_final(const Params p, int* __restrict__ labels, uint32_t* __restrict__ spins_w
             const int i = y * L + x;
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
-                if (j > 0 && vv[j] == vv[j - 1]) { ww[j] = ww[j - 1]; st[j] = st[j - 1]; }
-                else if (MODE == MODE_SW) {
-                    int l = ly * TW + 4 * lane + j;      // my own slot if I am an anchor
-                    int w = vv[j];
-                    if (!((anchor >> (4 * r + j)) & 1u)) {
-                        l = tile_local(p, vv[j], base, tw_eff, th_eff);   // >= 0: non-anchors point into the tile
-                        w = sm.S[l];
-                        const int lw = tile_local(p, w, base, tw_eff, th_eff);
-                        if (lw >= 0) l = lw;             // root inside the tile: its own slot; else the hooked local root's
-                    }
+                if (j > 0 && vv[j] == vv[j - 1] && vv[j] < 0) { ww[j] = ww[j - 1]; st[j] = st[j - 1]; }
+                else {
+                    int l = lb + j, w = vv[j];
+                    while (w < 0) { l = w & LMASK; w = sm.S[l]; }
                     ww[j] = w;
-                    st[j] = sm.st[l];
-                } else {
-                    const int l = tile_local(p, vv[j], base, tw_eff, th_eff);
-                    ww[j] = l >= 0 ? sm.S[l] : vv[j];
-                    st[j] = 0;
+                    st[j] = MODE == MODE_SW ? sm.st[l] : 0u;
                 }
                 nroots += (ww[j] == i + j);
             }
@@ -452,8 +494,8 @@ k_final(const Params p, int* __restrict__ labels, uint32_t* __restrict__ spins_w
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
-        nroots += __shfl_xor_sync(0xffffffffu, nroots, o);
-        if (MODE == MODE_WOLFF) nflip += __shfl_xor_sync(0xffffffffu, nflip, o);
+        nroots += __shfl_xor_sync(FULLM, nroots, o);
+        if (MODE == MODE_WOLFF) nflip += __shfl_xor_sync(FULLM, nflip, o);
     }
     if (lane == 0) {
         if (nroots) atomicAdd(&acc->n_clusters, (unsigned long long)nroots);

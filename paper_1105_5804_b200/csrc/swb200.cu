@@ -110,24 +110,21 @@ inline void prof_mark(sw_handle* h, int phase, cudaStream_t s)
 inline int grid_for(int64_t n, int block) { return (int)((n + block - 1) / block); }
 inline int grid_capped(int64_t n, int block, int cap) { int g = grid_for(n, block); return g < cap ? (g < 1 ? 1 : g) : cap; }
 
-// labelling of the bond graph of step t (or of packed bonds): k_local -> k_seam -> k_seamfix
+// labelling of the bond graph of step t (or of packed bonds): k_scan -> k_seam; k_final resolves the rest
 template <bool FROM_BONDS>
 int launch_label_front(sw_handle* h, const Params& p, const uint8_t* bonds, int32_t* labels, cudaStream_t s)
 {
-    const dim3 grid(p.ntx, p.nty);
     uint8_t* seamE = h->d_seam;
     uint8_t* seamN = h->d_seam + (size_t)p.ntx * p.L;
     prof_mark(h, 0, s);
-    k_local<FROM_BONDS><<<grid, NTHREADS, 0, s>>>(p, h->d_spins, bonds, labels, seamE, seamN, h->d_acc);
-    SW_LAUNCHED(h, "k_local");
+    k_scan<FROM_BONDS><<<dim3((p.ntx + SCAN_WARPS - 1) / SCAN_WARPS, p.nty), SCAN_THREADS, 0, s>>>(
+        p, h->d_spins, bonds, labels, seamE, seamN, h->d_acc);
+    SW_LAUNCHED(h, "k_scan");
     prof_mark(h, 1, s);
     const int nseam = (p.ntx + p.nty) * p.L;
     k_seam<<<grid_for(nseam, 256), 256, 0, s>>>(p, h->d_seam, labels);
     SW_LAUNCHED(h, "k_seam");
     prof_mark(h, 2, s);
-    k_seamfix<<<grid_for(nseam, 256), 256, 0, s>>>(p, h->d_seam, labels);
-    SW_LAUNCHED(h, "k_seamfix");
-    prof_mark(h, 3, s);
     return SW_OK;
 }
 
@@ -171,7 +168,6 @@ int sw_create(sw_handle** out, int32_t L, int32_t q, double beta, uint64_t seed)
     p.logL = -1;
     for (int k = 2; k <= 15; ++k) if ((1 << k) == L) p.logL = k;
     p.ntx = (L + TW - 1) / TW; p.nty = (L + TH - 1) / TH;
-    p.divL = ((1ull << 40) + (uint64_t)L - 1) / (uint64_t)L;
     const uint32_t s_lo = (uint32_t)(seed & 0xFFFFFFFFu), s_hi = (uint32_t)(seed >> 32);
     for (int r = 0; r < 10; ++r) {
         p.k0[r] = s_lo + (uint32_t)r * 0x9E3779B9u;
@@ -246,9 +242,6 @@ int sw_bind(sw_handle* h, void* d_spins, int32_t* d_labels, uint8_t* d_bonds, vo
     h->d_size = (int32_t*)(h->d_work + w.size);
     h->bound = false;
     h->have_labels = false;
-    SW_CUDA(h, cudaFuncSetAttribute(k_final<MODE_SW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FinalSmem)));
-    SW_CUDA(h, cudaFuncSetAttribute(k_final<MODE_WOLFF>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FinalSmem)));
-    SW_CUDA(h, cudaFuncSetAttribute(k_final<MODE_LABEL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FinalSmem)));
     SW_CUDA(h, cudaMemsetAsync(h->d_work, 0, w.seam, (cudaStream_t)stream));
     h->bound = true;
     return SW_OK;
@@ -281,9 +274,9 @@ int sw_sweep(sw_handle* h, int64_t n, void* stream)
         if (rc) return rc;
         rc = launch_label_front<false>(h, p, nullptr, h->d_labels, s);
         if (rc) return rc;
-        k_final<MODE_SW><<<dim3(p.ntx, p.nty), NTHREADS, sizeof(FinalSmem), s>>>(p, h->d_labels, h->d_spins, h->d_acc, nullptr);
+        k_final<MODE_SW><<<dim3(p.ntx, p.nty), FIN_THREADS, 0, s>>>(p, h->d_labels, h->d_spins, h->d_acc, nullptr);
         SW_LAUNCHED(h, "k_final<SW>");
-        prof_mark(h, 4, s);
+        prof_mark(h, 3, s);
         if (h->prof_on && h->prof_n < PROF_MAX) ++h->prof_n;
         ++h->t;
         h->have_labels = true;
@@ -315,9 +308,9 @@ int sw_label(sw_handle* h, const uint8_t* d_bonds_in, int32_t* d_labels_out, voi
     if (rc) return rc;
     rc = launch_label_front<true>(h, p, bonds, labels, s);
     if (rc) return rc;
-    k_final<MODE_LABEL><<<dim3(p.ntx, p.nty), NTHREADS, sizeof(int) * TW * TH, s>>>(p, labels, nullptr, h->d_acc, nullptr);
+    k_final<MODE_LABEL><<<dim3(p.ntx, p.nty), FIN_THREADS, 0, s>>>(p, labels, nullptr, h->d_acc, nullptr);
     SW_LAUNCHED(h, "k_final<LABEL>");
-    prof_mark(h, 4, s);
+    prof_mark(h, 3, s);
     if (h->prof_on && h->prof_n < PROF_MAX) ++h->prof_n;
     if (labels == h->d_labels) h->have_labels = true;
     return SW_OK;
@@ -370,10 +363,10 @@ int wolff_step(sw_handle* h, int64_t n, int64_t* h_sizes, void* stream)
             if (rc) return rc;
             rc = launch_label_front<false>(h, p, nullptr, h->d_labels, s);
             if (rc) return rc;
-            k_final<MODE_WOLFF><<<dim3(p.ntx, p.nty), NTHREADS, sizeof(int) * TW * TH, s>>>(p, h->d_labels, h->d_spins, h->d_acc,
+            k_final<MODE_WOLFF><<<dim3(p.ntx, p.nty), FIN_THREADS, 0, s>>>(p, h->d_labels, h->d_spins, h->d_acc,
                                                                          h->d_wolff + k);
             SW_LAUNCHED(h, "k_final<WOLFF>");
-            prof_mark(h, 4, s);
+            prof_mark(h, 3, s);
             if (h->prof_on && h->prof_n < PROF_MAX) ++h->prof_n;
             ++h->t;
             h->have_labels = true;

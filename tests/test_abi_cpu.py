@@ -94,7 +94,7 @@ def test_workspace_bytes_and_strerror(lib):
     assert lib.sw_workspace_bytes(6, 2) == 0 and lib.sw_workspace_bytes(64, 9) == 0
     for L in (4, 64, 100, 1024, 16384):
         wb = lib.sw_workspace_bytes(L, 2)
-        ntx, nty = -(-L // 128), -(-L // 64)
+        ntx, nty = -(-L // 128), -(-L // 32)
         assert wb >= 4 * L * L + (ntx + nty) * L
         assert wb < 4 * L * L + (ntx + nty) * L + 65536
     assert lib.sw_strerror(0) == b"ok"
