@@ -8,8 +8,8 @@
 // Design notes and the differences from the paper's kernels (self-labelling, hierarchical sewing) are in DESIGN.md.
 //
 // Provisional label array `prov` (the caller's int32 labels buffer) between k_scan and k_final:
-//   entry < 0  : REF | l  -- reference to the site with strip-local index l = ly * TW + lx of the SAME strip, l smaller
-//                than the site's own local index (a forest inside the strip)
+//   entry < 0  : REF | l  -- the site's strip-local ROOT is the site with strip-local index l = ly * TW + lx of the
+//                SAME strip, l smaller than the site's own local index (k_scan flattens its forest before it writes)
 //   entry >= 0 : global site index g <= own index; g == own index: the site is the root of its tree.  Only
 //                strip-local roots carry entries >= 0; k_seam hooks them to roots of other strips (always to a smaller
 //                global index), so the root of every tree is the minimum site index of its cluster.
@@ -26,41 +26,73 @@ constexpr unsigned FULLM = 0xffffffffu;
 __device__ __forceinline__ int strip_gidx(int base, int L, int l) { return base + (l >> TW_LOG) * L + (l & (TW - 1)); }
 
 // ------------------------------------------------------------------------------------------------ k_scan
-// find with path halving in the strip's node table (uint16 parent per strip-local site index; only node entries are
-// ever written or read).  Plain loads/stores: the table is private to one warp, see the 3-phase protocol below.
-__device__ __forceinline__ int tbl_find(volatile uint16_t* tbl, int x)
+// The strip's forest: one uint16 per strip-local site index.  Entry of a node = its parent node (itself: root); entry
+// of any other site = the name (node) it adopted.  Private to one warp.
+//
+// find with path halving over node entries.  Plain loads/stores, see the 3-phase protocol in unite_batch.
+__device__ __forceinline__ int nm_find(volatile uint16_t* nm, int x)
 {
-    int p = tbl[x];
+    int p = nm[x];
     while (p != x) {
-        const int gp = tbl[p];
+        const int gp = nm[p];
         if (gp == p) return p;
-        tbl[x] = (uint16_t)gp;
+        nm[x] = (uint16_t)gp;
         x = gp;
-        p = tbl[x];
+        p = nm[x];
     }
     return x;
 }
 
+// Unite up to 32 queued pairs of names, one per lane (pair = a << 16 | b), hooking the larger root under the smaller.
+// 3-phase protocol, no atomics (the forest belongs to this warp): (1) all lanes find roots -- nobody hooks, so a root
+// stays a root; (2) hook with a plain store -- lanes hooking the same root collide, one store wins; (3) re-read: losers
+// retry from the new roots.
+__device__ __forceinline__ void unite_batch(volatile uint16_t* nm, bool have, uint32_t pair)
+{
+    int ua = (int)(pair >> 16), ub = (int)(pair & 0xFFFFu);
+    while (__any_sync(FULLM, have)) {
+        if (have) {
+            ua = nm_find(nm, ua);
+            ub = nm_find(nm, ub);
+            if (ua == ub) have = false;
+            else if (ua < ub) { const int t = ua; ua = ub; ub = t; }
+        }
+        __syncwarp();
+        if (have) nm[ua] = (uint16_t)ub;
+        __syncwarp();
+        if (have && nm[ua] == ub) have = false;
+    }
+}
+
+constexpr int QCAP = 32 + TW;                            // < 32 pairs carried over + at most one new pair per site of a row
+
 // One warp per TW x TH strip, lane -> 4 consecutive columns, rows in sequence.  FROM_BONDS=false: read spins, draw
-// bonds (a1).  FROM_BONDS=true: read packed bonds (sw_label).  Writes the forest described above, the bonds that
-// cross the strip's east / north edge into seamE / seamN (one byte per seam site), and adds the number of active
-// bonds to acc->n_active.
+// bonds (a1).  FROM_BONDS=true: read packed bonds (sw_label).  Writes the flattened strip-local labelling described
+// above, the bonds that cross the strip's east / north edge into seamE / seamN (one byte per seam site), and adds the
+// number of active bonds to acc->n_active.
 //
-// Row step.  A "node" is a horizontal run (inside the strip) that has no active north bond from the row above; it is
-// named by its first site.  Every other run adopts the name carried by its leftmost contact with the row above, so
-// all sites written are either nodes or references to nodes.  Only when a run has further contacts whose names
-// differ from the adopted one, the two names are united in the node table (hooking the larger index under the
-// smaller).  The strip-local root is therefore the minimum site index of the strip-local component.
+// Pass 1, row by row.  A "node" is a horizontal run (inside the strip) that has no active north bond from the row
+// above; it is named by its first site.  Every other run adopts the name carried by its leftmost contact with the row
+// above, so every name is a node.  When a run has further contacts whose names differ from the adopted one, the pair
+// of names is queued; queued pairs are united 32 at a time (all lanes busy) in the strip's forest.  Names never depend
+// on the forest, so the row loop has no divergent part.
+// Pass 2, row by row: every site looks up the root of its name (the rows above are already flat, so this is one load
+// unless the name is a node of the same row), the row's entries are overwritten by their roots, and the row is written
+// to `prov` as REF | root (or the site's global index if it is the root: hooking is larger-under-smaller, so the root
+// is the minimum site index of the strip-local component).
 template <bool FROM_BONDS>
 __global__ void __launch_bounds__(SCAN_THREADS)
 k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __restrict__ bonds_in, int* prov,
        uint8_t* __restrict__ seamE, uint8_t* __restrict__ seamN, Acc* __restrict__ acc)
 {
-    __shared__ uint16_t s_tbl[SCAN_WARPS][TW * TH];
+    __shared__ __align__(16) uint16_t s_nm[SCAN_WARPS][TW * TH];
+    __shared__ uint32_t s_q[SCAN_WARPS][QCAP];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int tx = blockIdx.x * SCAN_WARPS + warp, ty = blockIdx.y;
     if (tx >= p.ntx) return;                             // no block-wide barrier in this kernel
-    volatile uint16_t* tbl = s_tbl[warp];
+    uint16_t* nm = s_nm[warp];
+    volatile uint16_t* vnm = nm;
+    volatile uint32_t* q = s_q[warp];
     const int L = p.L, Lw = L >> 2;
     const int x0 = tx * TW, y0 = ty * TH;
     const int tw_eff = min(TW, L - x0), th_eff = min(TH, L - y0);
@@ -68,7 +100,6 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
     const bool colv = 4 * lane < tw_eff;
     const int last_lane = (tw_eff >> 2) - 1;             // lane that owns the strip's last column
     const bool is_last = lane == last_lane;
-    const int base = y0 * L + x0;
     const int xw = x >> 2;
     const int xew = ((x + 4 == L) ? 0 : x + 4) >> 2;     // east halo word of the last lane (periodic)
     const unsigned lt = lanemask_lt(), me = 1u << lane, le = lt | me, gt = ~le;
@@ -89,6 +120,7 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
     int Lp0 = NONE, Lp1 = NONE, Lp2 = NONE, Lp3 = NONE;  // names carried by the previous row's sites
     uint32_t np = 0;                                     // active north bonds from the previous row into this row
     int nact = 0;
+    int qn = 0;                                          // queued pairs (warp-uniform)
 
     for (int ly = 0; ly < th_eff; ++ly) {
         const int y = y0 + ly;
@@ -184,62 +216,81 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
         if (useP) { l0 = RP; if (s1 == 0) l1 = RP; if (s2 == 0) l2 = RP; }
         if (useS) { l3 = RS; if (s2 == s3) l2 = RS; if (s1 == s3) l1 = RS; if (s3 == 0) l0 = RS; }
 
-        // new nodes of this row: root entries in the table (the global entry is written with the row below)
-        const bool new0 = l0 == ref0, new1 = l1 == ref0 + 1, new2 = l2 == ref0 + 2, new3 = l3 == ref0 + 3;
-        {
-            const int lb = ly * TW + 4 * lane;
-            if (new0) tbl[lb] = (uint16_t)lb;
-            if (new1) tbl[lb + 1] = (uint16_t)(lb + 1);
-            if (new2) tbl[lb + 2] = (uint16_t)(lb + 2);
-            if (new3) tbl[lb + 3] = (uint16_t)(lb + 3);
+        // the row's entries in the forest: a new node's name is its own index, i.e. it starts as a root
+        if (colv) {
+            uint2 o;
+            o.x = ((uint32_t)l0 & 0xFFFFu) | ((uint32_t)l1 << 16);
+            o.y = ((uint32_t)l2 & 0xFFFFu) | ((uint32_t)l3 << 16);
+            *reinterpret_cast<uint2*>(nm + ly * TW + 4 * lane) = o;
         }
 
-        // contacts whose carried name differs from the adopted one: unite the two trees.
-        // 3-phase protocol, no atomics (the table belongs to this warp): (1) all lanes find roots -- nobody hooks, so
-        // a root stays a root; (2) hook larger under smaller with a plain store -- lanes hooking the same root
-        // collide, one store wins; (3) re-read: losers retry.  Every successful hook is written through to `prov`.
+        // contacts whose carried name differs from the adopted one: queue the pair of names
         unsigned um = ((np & 1u) && Lp0 != l0 ? 1u : 0u) | ((np & 2u) && Lp1 != l1 ? 2u : 0u) |
                       ((np & 4u) && Lp2 != l2 ? 4u : 0u) | ((np & 8u) && Lp3 != l3 ? 8u : 0u);
-        if (__any_sync(FULLM, um != 0)) {
-            int ua = 0, ub = 0;
-            bool have = false;
-            while (true) {
-                if (!have && um) {
-                    const int c = __ffs(um) - 1;
-                    um &= um - 1;
-                    ua = (c == 0 ? Lp0 : c == 1 ? Lp1 : c == 2 ? Lp2 : Lp3) & LMASK;
-                    ub = (c == 0 ? l0 : c == 1 ? l1 : c == 2 ? l2 : l3) & LMASK;
-                    have = true;
-                }
-                if (!__any_sync(FULLM, have)) break;
-                __syncwarp();
-                if (have) {
-                    ua = tbl_find(tbl, ua);
-                    ub = tbl_find(tbl, ub);
-                    if (ua == ub) have = false;
-                    else if (ua < ub) { const int t = ua; ua = ub; ub = t; }
-                }
-                __syncwarp();
-                if (have) tbl[ua] = (uint16_t)ub;
-                __syncwarp();
-                if (have && tbl[ua] == ub) {
-                    prov[strip_gidx(base, L, ua)] = REF | ub;
-                    have = false;
-                }
+        unsigned B = __ballot_sync(FULLM, um != 0);
+        while (B) {
+            if (um) {
+                const int c = __ffs(um) - 1;
+                um &= um - 1;
+                const uint32_t ua = (uint32_t)(c == 0 ? Lp0 : c == 1 ? Lp1 : c == 2 ? Lp2 : Lp3) & 0xFFFFu;
+                const uint32_t ub = (uint32_t)(c == 0 ? l0 : c == 1 ? l1 : c == 2 ? l2 : l3) & 0xFFFFu;
+                q[qn + __popc(B & lt)] = (ua << 16) | ub;
             }
+            qn += __popc(B);
+            B = __ballot_sync(FULLM, um != 0);
+        }
+        if (qn >= 32) {
+            __syncwarp();                                // queue and row entries visible to the whole warp
+            do {
+                qn -= 32;
+                unite_batch(vnm, true, q[qn + lane]);
+            } while (qn >= 32);
         }
 
-        if (colv) {
-            const int gi = y * L + x;
-            int4 o;
-            o.x = new0 ? gi : l0;
-            o.y = new1 ? gi + 1 : l1;
-            o.z = new2 ? gi + 2 : l2;
-            o.w = new3 ? gi + 3 : l3;
-            *reinterpret_cast<int4*>(prov + (size_t)gi) = o;
-        }
         Lp0 = l0; Lp1 = l1; Lp2 = l2; Lp3 = l3;
         np = n4;
+    }
+
+    __syncwarp();
+    if (qn > 0) {
+        const bool have = lane < qn;
+        unite_batch(vnm, have, have ? q[lane] : 0u);
+    }
+    __syncwarp();
+
+    // ---- pass 2: flatten row by row and write the strip's labels ------------------------------------------------
+    for (int ly = 0; ly < th_eff; ++ly) {
+        const int lb = ly * TW + 4 * lane;
+        const int rowb = ly * TW;
+        int r0 = 0, r1 = 0, r2 = 0, r3 = 0;
+        if (colv) {
+            const uint2 v = *reinterpret_cast<const uint2*>(nm + lb);
+            const int n0 = v.x & 0xFFFFu, n1 = v.x >> 16, n2 = v.y & 0xFFFFu, n3 = v.y >> 16;
+            // names of the rows above are flat already: one load; a node of this row may be hooked anywhere: chase
+            r0 = vnm[n0];
+            if (n0 >= rowb) { int t = vnm[r0]; while (t != r0) { r0 = t; t = vnm[r0]; } }
+            if (n1 == n0) r1 = r0;
+            else { r1 = vnm[n1]; if (n1 >= rowb) { int t = vnm[r1]; while (t != r1) { r1 = t; t = vnm[r1]; } } }
+            if (n2 == n1) r2 = r1;
+            else { r2 = vnm[n2]; if (n2 >= rowb) { int t = vnm[r2]; while (t != r2) { r2 = t; t = vnm[r2]; } } }
+            if (n3 == n2) r3 = r2;
+            else { r3 = vnm[n3]; if (n3 >= rowb) { int t = vnm[r3]; while (t != r3) { r3 = t; t = vnm[r3]; } } }
+        }
+        __syncwarp();                                    // all reads of this row's entries done before they change
+        if (colv) {
+            uint2 o;
+            o.x = (uint32_t)r0 | ((uint32_t)r1 << 16);
+            o.y = (uint32_t)r2 | ((uint32_t)r3 << 16);
+            *reinterpret_cast<uint2*>(nm + lb) = o;
+            const int gi = (y0 + ly) * L + x;
+            int4 g;
+            g.x = r0 == lb ? gi : (REF | r0);
+            g.y = r1 == lb + 1 ? gi + 1 : (REF | r1);
+            g.z = r2 == lb + 2 ? gi + 2 : (REF | r2);
+            g.w = r3 == lb + 3 ? gi + 3 : (REF | r3);
+            *reinterpret_cast<int4*>(prov + (size_t)gi) = g;
+        }
+        __syncwarp();                                    // the flat entries are visible to the next row
     }
 
     if (!FROM_BONDS) {
@@ -473,7 +524,7 @@ k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __rest
                 if (j > 0 && vv[j] == vv[j - 1] && vv[j] < 0) { ww[j] = ww[j - 1]; st[j] = st[j - 1]; }
                 else {
                     int l = lb + j, w = vv[j];
-                    while (w < 0) { l = w & LMASK; w = sm.S[l]; }
+                    if (w < 0) { l = w & LMASK; w = sm.S[l]; }     // k_scan wrote flat references: one hop
                     ww[j] = w;
                     st[j] = MODE == MODE_SW ? sm.st[l] : 0u;
                 }
