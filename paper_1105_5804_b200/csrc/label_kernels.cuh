@@ -1,24 +1,28 @@
 // label_kernels.cuh -- the Swendsen-Wang hot path (S:8a rows a1-a5, a7):
 //   k_scan  : bond activation (P:53 step 1, Eq. 7) fused with strip-local labelling: one warp scans a
-//             TW x TH strip row by row, the labels of the previous row stay in registers, a run adopts the label of
-//             its first contact with the row above, and a (rare) union in a small shared-memory forest happens only
-//             when two different trees meet
+//             TW x TH strip row by row, the names of the previous row stay in registers, a run adopts the name of its
+//             first contact with the row above; pairs of names that meet are queued and united 32 at a time in a small
+//             shared-memory forest.  The roots of the strip's edge sites go to compact edge arrays.
 //   k_seam  : cross-strip consolidation as ONE concurrent union-find pass over the seam bonds
 //   k_final : flatten to canonical labels + cluster flip (P:55 step 3) / Wolff flip / label only
 // Design notes and the differences from the paper's kernels (self-labelling, hierarchical sewing) are in DESIGN.md.
 //
-// Provisional label array `prov` (the caller's int32 labels buffer) between k_scan and k_final:
-//   entry < 0  : REF | l  -- the site's strip-local ROOT is the site with strip-local index l = ly * TW + lx of the
-//                SAME strip, l smaller than the site's own local index (k_scan flattens its forest before it writes)
-//   entry >= 0 : global site index g <= own index; g == own index: the site is the root of its tree.  Only
-//                strip-local roots carry entries >= 0; k_seam hooks them to roots of other strips (always to a smaller
-//                global index), so the root of every tree is the minimum site index of its cluster.
+// Provisional label array `prov` (the caller's int32 labels buffer) between k_scan and k_final.  A "node" is a site
+// that names a run (see k_scan); every strip-local tree is a tree of nodes.
+//   entry >= 0            : the site is a node and the root of its strip-local tree; the value is a global site index
+//                           g <= own index (g == own index: root of its global tree; k_seam hooks roots of different
+//                           strips, always under a smaller global index, so the root of every tree is the minimum site
+//                           index of its cluster)
+//   entry = REF|HOOK|l    : the site is a node that was hooked under the node with strip-local index l < own
+//   entry = REF|l         : the site is not a node; it belongs to the tree of the node with strip-local index l
+// with l = ly * TW + lx inside the SAME strip.
 #pragma once
 #include "common.cuh"
 
 namespace swb {
 
 constexpr int REF = (int)0x80000000;
+constexpr int HOOK = 0x40000000;
 constexpr int LMASK = TW * TH - 1;
 constexpr int NONE = 0x7FFFFFFF;                         // "no contact" (any value >= 0 works)
 constexpr unsigned FULLM = 0xffffffffu;
@@ -27,9 +31,11 @@ __device__ __forceinline__ int strip_gidx(int base, int L, int l) { return base 
 
 // ------------------------------------------------------------------------------------------------ k_scan
 // The strip's forest: one uint16 per strip-local site index.  Entry of a node = its parent node (itself: root); entry
-// of any other site = the name (node) it adopted.  Private to one warp.
+// of any other site = the name (node) it adopted, so a chase that starts at any site ends at the root of its tree.
+// Private to one warp.
 //
-// find with path halving over node entries.  Plain loads/stores, see the 3-phase protocol in unite_batch.
+// find with path halving.  Roots change only through the atomicCAS in unite_batch; halving rewrites non-root entries
+// with an ancestor (plain store: concurrent lanes may interleave, every value written is an ancestor).
 __device__ __forceinline__ int nm_find(volatile uint16_t* nm, int x)
 {
     int p = nm[x];
@@ -43,47 +49,54 @@ __device__ __forceinline__ int nm_find(volatile uint16_t* nm, int x)
     return x;
 }
 
-// Unite up to 32 queued pairs of names, one per lane (pair = a << 16 | b), hooking the larger root under the smaller.
-// 3-phase protocol, no atomics (the forest belongs to this warp): (1) all lanes find roots -- nobody hooks, so a root
-// stays a root; (2) hook with a plain store -- lanes hooking the same root collide, one store wins; (3) re-read: losers
-// retry from the new roots.
-__device__ __forceinline__ void unite_batch(volatile uint16_t* nm, bool have, uint32_t pair)
+__device__ __forceinline__ int nm_root(const volatile uint16_t* nm, int x)
+{
+    int p = nm[x];
+    while (p != x) { x = p; p = nm[x]; }
+    return x;
+}
+
+// Unite one queued pair of names per lane (pair = a << 16 | b): hook the larger root under the smaller with a 16-bit
+// compare-and-swap (it succeeds only while the larger one still is a root; otherwise retry from the new roots) and
+// write the hook through to `prov`.
+__device__ __forceinline__ void unite_batch(volatile uint16_t* nm, bool have, uint32_t pair, int* prov, int base, int L)
 {
     int ua = (int)(pair >> 16), ub = (int)(pair & 0xFFFFu);
-    while (__any_sync(FULLM, have)) {
-        if (have) {
-            ua = nm_find(nm, ua);
-            ub = nm_find(nm, ub);
-            if (ua == ub) have = false;
-            else if (ua < ub) { const int t = ua; ua = ub; ub = t; }
+    while (have) {
+        ua = nm_find(nm, ua);
+        ub = nm_find(nm, ub);
+        if (ua == ub) break;
+        if (ua < ub) { const int t = ua; ua = ub; ub = t; }
+        const unsigned short old = atomicCAS(const_cast<unsigned short*>(reinterpret_cast<volatile unsigned short*>(nm)) + ua,
+                                             (unsigned short)ua, (unsigned short)ub);
+        if (old == (unsigned short)ua) {
+            prov[strip_gidx(base, L, ua)] = REF | HOOK | ub;
+            break;
         }
-        __syncwarp();
-        if (have) nm[ua] = (uint16_t)ub;
-        __syncwarp();
-        if (have && nm[ua] == ub) have = false;
     }
 }
 
 constexpr int QCAP = 32 + TW;                            // < 32 pairs carried over + at most one new pair per site of a row
 
-// One warp per TW x TH strip, lane -> 4 consecutive columns, rows in sequence.  FROM_BONDS=false: read spins, draw
-// bonds (a1).  FROM_BONDS=true: read packed bonds (sw_label).  Writes the flattened strip-local labelling described
-// above, the bonds that cross the strip's east / north edge into seamE / seamN (one byte per seam site), and adds the
-// number of active bonds to acc->n_active.
+// Edge arrays (workspace): for every site on the edge of a strip the global index of its strip-local root.
+//   edgeA = [ rootE (ntx * L) | rootN (nty * L) ] : last column of strip column tc at row y -> [tc * L + y], last row of
+//           strip row tr at column x -> [ntx * L + tr * L + x]; the value is -1 if the bond that leaves the strip there
+//           (east bond of the last column, north bond of the last row) is not active
+//   edgeB = [ rootW (ntx * L) | rootS (nty * L) ] : first column / first row, same indexing
 //
-// Pass 1, row by row.  A "node" is a horizontal run (inside the strip) that has no active north bond from the row
-// above; it is named by its first site.  Every other run adopts the name carried by its leftmost contact with the row
-// above, so every name is a node.  When a run has further contacts whose names differ from the adopted one, the pair
-// of names is queued; queued pairs are united 32 at a time (all lanes busy) in the strip's forest.  Names never depend
-// on the forest, so the row loop has no divergent part.
-// Pass 2, row by row: every site looks up the root of its name (the rows above are already flat, so this is one load
-// unless the name is a node of the same row), the row's entries are overwritten by their roots, and the row is written
-// to `prov` as REF | root (or the site's global index if it is the root: hooking is larger-under-smaller, so the root
-// is the minimum site index of the strip-local component).
+// One warp per TW x TH strip, lane -> 4 consecutive columns, rows in sequence.  FROM_BONDS=false: read spins, draw
+// bonds (a1).  FROM_BONDS=true: read packed bonds (sw_label).  Writes the provisional labels described above and the
+// edge arrays, and adds the number of active bonds to acc->n_active.
+//
+// Row step.  A "node" is a horizontal run (inside the strip) that has no active north bond from the row above; it is
+// named by its first site.  Every other run adopts the name carried by its leftmost contact with the row above, so
+// every name is a node.  When a run has further contacts whose names differ from the adopted one, the pair of names is
+// queued; queued pairs are united 32 at a time (all lanes busy) in the strip's forest.  Names never depend on the
+// forest, so the row loop has no divergent part.
 template <bool FROM_BONDS>
 __global__ void __launch_bounds__(SCAN_THREADS)
 k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __restrict__ bonds_in, int* prov,
-       uint8_t* __restrict__ seamE, uint8_t* __restrict__ seamN, Acc* __restrict__ acc)
+       int* __restrict__ edgeA, int* __restrict__ edgeB, Acc* __restrict__ acc)
 {
     __shared__ __align__(16) uint16_t s_nm[SCAN_WARPS][TW * TH];
     __shared__ uint32_t s_q[SCAN_WARPS][QCAP];
@@ -100,6 +113,7 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
     const bool colv = 4 * lane < tw_eff;
     const int last_lane = (tw_eff >> 2) - 1;             // lane that owns the strip's last column
     const bool is_last = lane == last_lane;
+    const int base = y0 * L + x0;
     const int xw = x >> 2;
     const int xew = ((x + 4 == L) ? 0 : x + 4) >> 2;     // east halo word of the last lane (periodic)
     const unsigned lt = lanemask_lt(), me = 1u << lane, le = lt | me, gt = ~le;
@@ -121,6 +135,8 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
     uint32_t np = 0;                                     // active north bonds from the previous row into this row
     int nact = 0;
     int qn = 0;                                          // queued pairs (warp-uniform)
+    uint32_t eastm = 0;                                  // last lane: bit ly = the east bond that leaves the strip in row ly
+    uint32_t northm = 0;                                 // the 4 north bonds that leave the strip in the last row
 
     for (int ly = 0; ly < th_eff; ++ly) {
         const int y = y0 + ly;
@@ -158,16 +174,14 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
             n4 = ((b >> 1) & 1) | ((b >> 2) & 2) | ((b >> 3) & 4) | ((b >> 4) & 8);
         }
 
-        // bonds that leave the strip go to the seam arrays and are dropped here
-        if (colv) {
-            if (is_last) {
-                seamE[(size_t)tx * L + y] = (uint8_t)(e4 >> 3);
-                e4 &= 7u;
-            }
-            if (ly == th_eff - 1) {
-                *reinterpret_cast<uint32_t*>(seamN + (size_t)ty * L + x) = bits_to_bytes4(n4);
-                n4 = 0;
-            }
+        // bonds that leave the strip are remembered for the edge arrays and dropped here
+        if (is_last) {
+            eastm |= (e4 >> 3) << ly;
+            e4 &= 7u;
+        }
+        if (ly == th_eff - 1) {
+            northm = n4;
+            n4 = 0;
         }
 
         // ---- names of this row's sites ----------------------------------------------------------------------
@@ -216,35 +230,43 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
         if (useP) { l0 = RP; if (s1 == 0) l1 = RP; if (s2 == 0) l2 = RP; }
         if (useS) { l3 = RS; if (s2 == s3) l2 = RS; if (s1 == s3) l1 = RS; if (s3 == 0) l0 = RS; }
 
-        // the row's entries in the forest: a new node's name is its own index, i.e. it starts as a root
+        // the row's entries in the forest (a new node's name is its own index, i.e. it starts as a root) and in `prov`
         if (colv) {
             uint2 o;
             o.x = ((uint32_t)l0 & 0xFFFFu) | ((uint32_t)l1 << 16);
             o.y = ((uint32_t)l2 & 0xFFFFu) | ((uint32_t)l3 << 16);
             *reinterpret_cast<uint2*>(nm + ly * TW + 4 * lane) = o;
+            const int gi = y * L + x;
+            int4 g;
+            g.x = l0 == ref0 ? gi : l0;
+            g.y = l1 == ref0 + 1 ? gi + 1 : l1;
+            g.z = l2 == ref0 + 2 ? gi + 2 : l2;
+            g.w = l3 == ref0 + 3 ? gi + 3 : l3;
+            *reinterpret_cast<int4*>(prov + (size_t)gi) = g;
         }
 
         // contacts whose carried name differs from the adopted one: queue the pair of names
-        unsigned um = ((np & 1u) && Lp0 != l0 ? 1u : 0u) | ((np & 2u) && Lp1 != l1 ? 2u : 0u) |
-                      ((np & 4u) && Lp2 != l2 ? 4u : 0u) | ((np & 8u) && Lp3 != l3 ? 8u : 0u);
-        unsigned B = __ballot_sync(FULLM, um != 0);
-        while (B) {
-            if (um) {
-                const int c = __ffs(um) - 1;
-                um &= um - 1;
-                const uint32_t ua = (uint32_t)(c == 0 ? Lp0 : c == 1 ? Lp1 : c == 2 ? Lp2 : Lp3) & 0xFFFFu;
-                const uint32_t ub = (uint32_t)(c == 0 ? l0 : c == 1 ? l1 : c == 2 ? l2 : l3) & 0xFFFFu;
-                q[qn + __popc(B & lt)] = (ua << 16) | ub;
-            }
-            qn += __popc(B);
-            B = __ballot_sync(FULLM, um != 0);
+        {
+            const bool m0 = (np & 1u) && Lp0 != l0, m1 = (np & 2u) && Lp1 != l1;
+            const bool m2 = (np & 4u) && Lp2 != l2, m3 = (np & 8u) && Lp3 != l3;
+            const unsigned B0 = __ballot_sync(FULLM, m0), B1 = __ballot_sync(FULLM, m1);
+            const unsigned B2 = __ballot_sync(FULLM, m2), B3 = __ballot_sync(FULLM, m3);
+            if (m0) q[qn + __popc(B0 & lt)] = __byte_perm((uint32_t)l0, (uint32_t)Lp0, 0x5410);
+            qn += __popc(B0);
+            if (m1) q[qn + __popc(B1 & lt)] = __byte_perm((uint32_t)l1, (uint32_t)Lp1, 0x5410);
+            qn += __popc(B1);
+            if (m2) q[qn + __popc(B2 & lt)] = __byte_perm((uint32_t)l2, (uint32_t)Lp2, 0x5410);
+            qn += __popc(B2);
+            if (m3) q[qn + __popc(B3 & lt)] = __byte_perm((uint32_t)l3, (uint32_t)Lp3, 0x5410);
+            qn += __popc(B3);
         }
         if (qn >= 32) {
-            __syncwarp();                                // queue and row entries visible to the whole warp
+            __syncwarp();                                // queue, forest entries and `prov` rows visible to the whole warp
             do {
                 qn -= 32;
-                unite_batch(vnm, true, q[qn + lane]);
+                unite_batch(vnm, true, q[qn + lane], prov, base, L);
             } while (qn >= 32);
+            __syncwarp();                                // queue slots read before the next row overwrites them
         }
 
         Lp0 = l0; Lp1 = l1; Lp2 = l2; Lp3 = l3;
@@ -254,43 +276,36 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
     __syncwarp();
     if (qn > 0) {
         const bool have = lane < qn;
-        unite_batch(vnm, have, have ? q[lane] : 0u);
+        unite_batch(vnm, have, have ? q[lane] : 0u, prov, base, L);
     }
     __syncwarp();
 
-    // ---- pass 2: flatten row by row and write the strip's labels ------------------------------------------------
-    for (int ly = 0; ly < th_eff; ++ly) {
-        const int lb = ly * TW + 4 * lane;
-        const int rowb = ly * TW;
-        int r0 = 0, r1 = 0, r2 = 0, r3 = 0;
+    // ---- edge arrays: strip-local roots of the sites on the four edges ----------------------------------------------
+    {
+        const int nE = p.ntx * L;
         if (colv) {
-            const uint2 v = *reinterpret_cast<const uint2*>(nm + lb);
-            const int n0 = v.x & 0xFFFFu, n1 = v.x >> 16, n2 = v.y & 0xFFFFu, n3 = v.y >> 16;
-            // names of the rows above are flat already: one load; a node of this row may be hooked anywhere: chase
-            r0 = vnm[n0];
-            if (n0 >= rowb) { int t = vnm[r0]; while (t != r0) { r0 = t; t = vnm[r0]; } }
-            if (n1 == n0) r1 = r0;
-            else { r1 = vnm[n1]; if (n1 >= rowb) { int t = vnm[r1]; while (t != r1) { r1 = t; t = vnm[r1]; } } }
-            if (n2 == n1) r2 = r1;
-            else { r2 = vnm[n2]; if (n2 >= rowb) { int t = vnm[r2]; while (t != r2) { r2 = t; t = vnm[r2]; } } }
-            if (n3 == n2) r3 = r2;
-            else { r3 = vnm[n3]; if (n3 >= rowb) { int t = vnm[r3]; while (t != r3) { r3 = t; t = vnm[r3]; } } }
+            // first row -> rootS, last row -> rootN (-1 where the north bond that leaves the strip is not active)
+            const int lb0 = 4 * lane, lb1 = (th_eff - 1) * TW + 4 * lane;
+            int4 s, n;
+            s.x = strip_gidx(base, L, nm_root(vnm, lb0));
+            s.y = strip_gidx(base, L, nm_root(vnm, lb0 + 1));
+            s.z = strip_gidx(base, L, nm_root(vnm, lb0 + 2));
+            s.w = strip_gidx(base, L, nm_root(vnm, lb0 + 3));
+            n.x = (northm & 1u) ? strip_gidx(base, L, nm_root(vnm, lb1)) : -1;
+            n.y = (northm & 2u) ? strip_gidx(base, L, nm_root(vnm, lb1 + 1)) : -1;
+            n.z = (northm & 4u) ? strip_gidx(base, L, nm_root(vnm, lb1 + 2)) : -1;
+            n.w = (northm & 8u) ? strip_gidx(base, L, nm_root(vnm, lb1 + 3)) : -1;
+            *reinterpret_cast<int4*>(edgeB + (size_t)nE + (size_t)ty * L + x) = s;
+            *reinterpret_cast<int4*>(edgeA + (size_t)nE + (size_t)ty * L + x) = n;
         }
-        __syncwarp();                                    // all reads of this row's entries done before they change
-        if (colv) {
-            uint2 o;
-            o.x = (uint32_t)r0 | ((uint32_t)r1 << 16);
-            o.y = (uint32_t)r2 | ((uint32_t)r3 << 16);
-            *reinterpret_cast<uint2*>(nm + lb) = o;
-            const int gi = (y0 + ly) * L + x;
-            int4 g;
-            g.x = r0 == lb ? gi : (REF | r0);
-            g.y = r1 == lb + 1 ? gi + 1 : (REF | r1);
-            g.z = r2 == lb + 2 ? gi + 2 : (REF | r2);
-            g.w = r3 == lb + 3 ? gi + 3 : (REF | r3);
-            *reinterpret_cast<int4*>(prov + (size_t)gi) = g;
+        // first column -> rootW, last column -> rootE: lane i takes row i
+        const uint32_t em = __shfl_sync(FULLM, eastm, last_lane);
+        if (lane < th_eff) {
+            const int w = strip_gidx(base, L, nm_root(vnm, lane * TW));
+            const int e = ((em >> lane) & 1u) ? strip_gidx(base, L, nm_root(vnm, lane * TW + tw_eff - 1)) : -1;
+            edgeB[(size_t)tx * L + y0 + lane] = w;
+            edgeA[(size_t)tx * L + y0 + lane] = e;
         }
-        __syncwarp();                                    // the flat entries are visible to the next row
     }
 
     if (!FROM_BONDS) {
@@ -301,34 +316,6 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
 }
 
 // ------------------------------------------------------------------------------------------------ seams
-// Seam site id -> the two end sites of its crossing bond and the origins of the strips they lie in.
-// ids [0, ntx*L): east seams (strip column tc, row y); ids [ntx*L, (ntx+nty)*L): north seams (strip row tr, column x).
-__device__ __forceinline__ void seam_sites(const Params& p, int id, int& a, int& b, int& base_a, int& base_b)
-{
-    const int L = p.L;
-    const int nE = p.ntx * L;
-    if (id < nE) {
-        const int tc = div_L(p, (uint32_t)id), y = id - tc * L;
-        const int xs = min((tc + 1) * TW, L) - 1;
-        const int xb = xs + 1 == L ? 0 : xs + 1;
-        const int yb0 = (y >> TH_LOG) << TH_LOG;
-        a = y * L + xs;
-        b = y * L + xb;
-        base_a = yb0 * L + tc * TW;
-        base_b = yb0 * L + xb;
-    } else {
-        const int k = id - nE;
-        const int tr = div_L(p, (uint32_t)k), x = k - tr * L;
-        const int ys = min((tr + 1) * TH, L) - 1;
-        const int yb = ys + 1 == L ? 0 : ys + 1;
-        const int xb0 = (x >> TW_LOG) << TW_LOG;
-        a = ys * L + x;
-        b = yb * L + x;
-        base_a = tr * TH * L + xb0;
-        base_b = yb * L + xb0;
-    }
-}
-
 // strip-local root (global index) of `site`: follow the strip-local references
 __device__ __forceinline__ int strip_root(const int* prov, int L, int site, int base)
 {
@@ -378,25 +365,34 @@ __device__ __forceinline__ void gunite(int* prov, int a, int b)
     }
 }
 
-// One thread per seam site: if its crossing bond is active, unite the strip-local roots of its two ends.
-// `seam` is seamE followed by seamN (contiguous).
+// One thread per seam site (ids [0, ntx*L): east seams (strip column tc, row y); then nty*L north seams (strip row tr,
+// column x)): if its crossing bond is active (edgeA >= 0), unite the strip-local roots of its two ends.
 __global__ void __launch_bounds__(256)
-k_seam(const Params p, const uint8_t* __restrict__ seam, int* prov)
+k_seam(const Params p, const int* __restrict__ edgeA, const int* __restrict__ edgeB, int* prov)
 {
-    const int nseam = (p.ntx + p.nty) * p.L;
+    const int L = p.L;
+    const int nE = p.ntx * L, nseam = (p.ntx + p.nty) * L;
     const int id = blockIdx.x * blockDim.x + threadIdx.x;
-    const bool on = id < nseam && seam[id];
     int ra = -1, rb = -1;
-    if (on) {
-        int a, b, base_a, base_b;
-        seam_sites(p, id, a, b, base_a, base_b);
-        ra = strip_root(prov, p.L, a, base_a);
-        rb = strip_root(prov, p.L, b, base_b);
+    if (id < nseam) {
+        ra = edgeA[id];
+        if (ra >= 0) {
+            int idb;
+            if (id < nE) {                               // first column of the strip column to the east (periodic)
+                const int tc = div_L(p, (uint32_t)id);
+                idb = tc + 1 == p.ntx ? id - tc * L : id + L;
+            } else {                                     // first row of the strip row to the north (periodic)
+                const int k = id - nE;
+                const int tr = div_L(p, (uint32_t)k);
+                idb = tr + 1 == p.nty ? id - tr * L : id + L;
+            }
+            rb = edgeB[idb];
+        }
     }
     // the previous seam site joins the same two strip-local clusters: skip (its thread does the union)
     const int pa = __shfl_up_sync(FULLM, ra, 1), pb = __shfl_up_sync(FULLM, rb, 1);
     const bool dup = (threadIdx.x & 31) != 0 && pa == ra && pb == rb;
-    if (on && !dup) gunite(prov, ra, rb);
+    if (ra >= 0 && !dup) gunite(prov, ra, rb);
 }
 
 // ------------------------------------------------------------------------------------------------ k_final
@@ -409,12 +405,13 @@ __device__ __forceinline__ uint32_t flip_state(const Params& p, int root)
     return __umulhi(w0, (uint32_t)p.q);                  // uniform state in [0,q)  (S:8c.6)
 }
 
-// Shared memory of k_final: the strip's forest, one state byte per strip-local root, the compacted list of roots.
+// Shared memory of k_final: the strip's entries (node entries are rewritten in place), one state byte per strip-local
+// root, and the compacted lists: strip-local roots from the front, hooked nodes from the back (together <= TW*TH).
 struct FinalSmem {
     int      S[TW * TH];
     uint16_t list[TW * TH];
     uint8_t  st[TW * TH];
-    int      nlist;
+    int      nroot, nhook;
     int      r0;
 };
 
@@ -422,12 +419,14 @@ struct FinalSmem {
 //   MODE_SW    : s_i = state drawn for the root (assign, P:55 step 3)
 //   MODE_WOLFF : s_i = -s_i iff root(i) == root(seed site i0); adds |C| to *wolff_size
 //   MODE_LABEL : labels only
-// Strip-local roots (entries >= 0) are compacted into a list; each is resolved to the root of its global tree (a
-// chase over entries >= 0 of other strips, which concurrently running CTAs may already have overwritten with final
-// labels -- those are roots of the same tree, so the chase still ends at the right root) and draws one Philox state.
-// Every other site follows its strip-local references through shared memory.
+// (1) the strip's entries go to shared memory; roots and hooked nodes are compacted into lists.  (2) every strip-local
+// root is resolved to the root of its global tree (a chase over entries >= 0 of other strips, which concurrently running
+// CTAs may already have overwritten with final labels -- those are roots of the same tree, so the chase still ends at the
+// right root) and draws one Philox state.  (3) every hooked node follows its references to the strip-local root and
+// then refers to it directly (concurrent rewrites only shorten paths).  (4) every site reaches its strip-local root in
+// at most two hops: own entry -> node -> root.
 template <int MODE>
-__global__ void __launch_bounds__(FIN_THREADS)
+__global__ void __launch_bounds__(FIN_THREADS, 7)
 k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __restrict__ acc,
         unsigned long long* __restrict__ wolff_size)
 {
@@ -443,7 +442,8 @@ k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __rest
     const int base = y0 * L + x0;
 
     if (threadIdx.x == 0) {
-        sm.nlist = 0;
+        sm.nroot = 0;
+        sm.nhook = 0;
         if (MODE == MODE_WOLFF) {
             uint32_t w0, w1, w2, w3;
             philox4x32_10(p, 0u, p.t_lo, p.t_hi, DOM_WSEED, w0, w1, w2, w3);
@@ -453,82 +453,96 @@ k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __rest
             sm.r0 = gfind(labels, strip_root(labels, L, i0, b0));
         }
     }
+    __syncthreads();                                     // counters (and r0) visible
 
-    uint32_t rootm = 0;                                  // bit 4r+j: my site (row r, column j) is a strip-local root
-#pragma unroll
-    for (int r = 0; r < R; ++r) {
-        const int ly = ly0 + r, y = y0 + ly;
-        if (y < L && colv) {
-            const int4 v = *reinterpret_cast<const int4*>(labels + (size_t)y * L + x);
-            *reinterpret_cast<int4*>(&sm.S[ly * TW + 4 * lane]) = v;
-            const int i = y * L + x;
-            if (MODE == MODE_SW)
-                rootm |= ((v.x >= 0) | ((v.y >= 0) << 1) | ((v.z >= 0) << 2) | ((v.w >= 0) << 3)) << (4 * r);
-            else                                         // only hooked roots need work
-                rootm |= ((v.x >= 0 && v.x != i) | ((v.y >= 0 && v.y != i + 1) << 1) | ((v.z >= 0 && v.z != i + 2) << 2) |
-                          ((v.w >= 0 && v.w != i + 3) << 3)) << (4 * r);
-        }
-    }
-    __syncthreads();                                     // nlist = 0, r0 and S visible
-
-    // compact the roots of the whole strip into sm.list (warp scan + one shared atomic per warp)
+    // (1) entries -> shared memory; compact roots (from the front of sm.list) and hooked nodes (from the back)
     {
-        const int cnt = __popc(rootm);
+        uint32_t rootm = 0, hookm = 0;                   // bit 4r+j: my site (row r, column j) is a root / a hooked node
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int ly = ly0 + r, y = y0 + ly;
+            if (y < L && colv) {
+                const int4 v = *reinterpret_cast<const int4*>(labels + (size_t)y * L + x);
+                *reinterpret_cast<int4*>(&sm.S[ly * TW + 4 * lane]) = v;
+                rootm |= ((v.x >= 0) | ((v.y >= 0) << 1) | ((v.z >= 0) << 2) | ((v.w >= 0) << 3)) << (4 * r);
+                constexpr int RH = REF | HOOK;
+                hookm |= (((v.x & RH) == RH) | (((v.y & RH) == RH) << 1) | (((v.z & RH) == RH) << 2) |
+                          (((v.w & RH) == RH) << 3)) << (4 * r);
+            }
+        }
+        const int cnt = __popc(rootm) | (__popc(hookm) << 16);
         int incl = cnt;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
             const int t = __shfl_up_sync(FULLM, incl, o);
             if (lane >= o) incl += t;
         }
-        int wbase = 0;
-        if (lane == 31 && incl) wbase = atomicAdd(&sm.nlist, incl);
-        wbase = __shfl_sync(FULLM, wbase, 31);
-        int pos = wbase + incl - cnt;
+        int rbase = 0, hbase = 0;
+        if (lane == 31) {
+            if (incl & 0xFFFF) rbase = atomicAdd(&sm.nroot, incl & 0xFFFF);
+            if (incl >> 16) hbase = atomicAdd(&sm.nhook, incl >> 16);
+        }
+        rbase = __shfl_sync(FULLM, rbase, 31);
+        hbase = __shfl_sync(FULLM, hbase, 31);
+        const int excl = incl - cnt;
+        int pos = rbase + (excl & 0xFFFF);
         for (uint32_t m = rootm; m; m &= m - 1) {
             const int b = __ffs(m) - 1;
             sm.list[pos++] = (uint16_t)((ly0 + (b >> 2)) * TW + 4 * lane + (b & 3));
         }
+        pos = TW * TH - 1 - (hbase + (excl >> 16));
+        for (uint32_t m = hookm; m; m &= m - 1) {
+            const int b = __ffs(m) - 1;
+            sm.list[pos--] = (uint16_t)((ly0 + (b >> 2)) * TW + 4 * lane + (b & 3));
+        }
     }
     __syncthreads();
-    // one global resolve + one Philox draw per strip-local root, balanced over the CTA
+    // (2) one global resolve + one Philox draw per strip-local root, (3) one chase per hooked node; both balanced over
+    // the CTA.  (3) only reads and writes references (< 0), (2) only root entries (>= 0), so they need no barrier
+    // between them.
+    int nroots = 0;
     {
-        const int n = sm.nlist;
+        const int n = sm.nroot;
         for (int k = threadIdx.x; k < n; k += FIN_THREADS) {
             const int l = sm.list[k];
             int v = sm.S[l];
-            if (v != strip_gidx(base, L, l)) {           // hooked by k_seam: find the root of the global tree
+            const int g = strip_gidx(base, L, l);
+            if (v != g) {                                // hooked by k_seam: find the root of the global tree
                 v = gfind(labels, v);
                 sm.S[l] = v;
             }
+            nroots += (v == g);
             if (MODE == MODE_SW) sm.st[l] = (uint8_t)flip_state(p, v);
+        }
+        const int nh = sm.nhook;
+        volatile int* S = sm.S;
+        for (int k = threadIdx.x; k < nh; k += FIN_THREADS) {
+            const int l = sm.list[TW * TH - 1 - k];
+            int r = S[l] & LMASK, e = S[r];
+            while (e < 0) { r = e & LMASK; e = S[r]; }
+            S[l] = REF | r;
         }
     }
     __syncthreads();
 
+    // (4) every site
     const int r0 = MODE == MODE_WOLFF ? sm.r0 : -1;
-    int nroots = 0, nflip = 0;
+    int nflip = 0;
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         const int ly = ly0 + r, y = y0 + ly;
         if (y < L && colv) {
             const int lb = ly * TW + 4 * lane;
             const int4 v = *reinterpret_cast<const int4*>(&sm.S[lb]);
-            const int vv[4] = {v.x, v.y, v.z, v.w};
-            int ww[4];
+            int ww[4] = {v.x, v.y, v.z, v.w};
             uint32_t st[4];
-            uint32_t old = 0;
-            if (MODE == MODE_WOLFF) old = spins_w[((size_t)y * L + x) >> 2];
-            const int i = y * L + x;
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
-                if (j > 0 && vv[j] == vv[j - 1] && vv[j] < 0) { ww[j] = ww[j - 1]; st[j] = st[j - 1]; }
-                else {
-                    int l = lb + j, w = vv[j];
-                    if (w < 0) { l = w & LMASK; w = sm.S[l]; }     // k_scan wrote flat references: one hop
-                    ww[j] = w;
-                    st[j] = MODE == MODE_SW ? sm.st[l] : 0u;
-                }
-                nroots += (ww[j] == i + j);
+                int l = lb + j, w = ww[j];
+                if (w < 0) { l = w & LMASK; w = sm.S[l]; }
+                if (w < 0) { l = w & LMASK; w = sm.S[l]; }
+                ww[j] = w;
+                st[j] = MODE == MODE_SW ? sm.st[l] : 0u;
             }
             *reinterpret_cast<int4*>(labels + (size_t)y * L + x) = make_int4(ww[0], ww[1], ww[2], ww[3]);
             if (MODE == MODE_SW) {
@@ -536,10 +550,13 @@ k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __rest
                 if (p.q == 2) word = 0x01010101u | (word * 0xFEu);   // k=0 -> +1 (0x01), k=1 -> -1 (0xFF)
                 spins_w[((size_t)y * L + x) >> 2] = word;
             } else if (MODE == MODE_WOLFF) {
-                uint32_t m = 0;                          // bytes to negate
-#pragma unroll
-                for (int j = 0; j < 4; ++j) if (ww[j] == r0) { m |= 0xFFu << (8 * j); ++nflip; }
-                if (m) spins_w[((size_t)y * L + x) >> 2] = __vneg4(old & m) | (old & ~m);
+                const uint32_t m = (ww[0] == r0 ? 0xFFu : 0u) | (ww[1] == r0 ? 0xFF00u : 0u) |
+                                   (ww[2] == r0 ? 0xFF0000u : 0u) | (ww[3] == r0 ? 0xFF000000u : 0u);   // bytes to negate
+                if (m) {
+                    const uint32_t old = spins_w[((size_t)y * L + x) >> 2];
+                    spins_w[((size_t)y * L + x) >> 2] = __vneg4(old & m) | (old & ~m);
+                    nflip += __popc(m) >> 3;
+                }
             }
         }
     }

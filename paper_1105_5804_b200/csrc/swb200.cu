@@ -29,7 +29,8 @@ struct sw_handle {
     // carved from d_work
     Acc*      d_acc;
     unsigned long long* d_wolff;   // WOLFF_RING slots
-    uint8_t*  d_seam;              // seamE (ntx*L) followed by seamN (nty*L)
+    int32_t*  d_edgeA;             // (ntx+nty)*L: strip-local roots of last columns / last rows (-1: bond inactive)
+    int32_t*  d_edgeB;             // (ntx+nty)*L: strip-local roots of first columns / first rows
     int32_t*  d_size;              // N int32
     bool      bound;
     bool      have_labels;         // a labelling has happened since bind
@@ -46,7 +47,7 @@ namespace {
 constexpr size_t ALIGN = 256;
 inline size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
-struct WorkLayout { size_t acc, wolff, seam, size, total; };
+struct WorkLayout { size_t acc, wolff, edgeA, edgeB, size, total; };
 
 WorkLayout work_layout(int32_t L)
 {
@@ -55,8 +56,9 @@ WorkLayout work_layout(int32_t L)
     WorkLayout w;
     w.acc = 0;
     w.wolff = align_up(sizeof(Acc));
-    w.seam = w.wolff + align_up(sizeof(unsigned long long) * WOLFF_RING);
-    w.size = w.seam + align_up((ntx + nty) * (size_t)L);
+    w.edgeA = w.wolff + align_up(sizeof(unsigned long long) * WOLFF_RING);
+    w.edgeB = w.edgeA + align_up((ntx + nty) * (size_t)L * sizeof(int32_t));
+    w.size = w.edgeB + align_up((ntx + nty) * (size_t)L * sizeof(int32_t));
     w.total = w.size + align_up(N * sizeof(int32_t));
     return w;
 }
@@ -114,15 +116,13 @@ inline int grid_capped(int64_t n, int block, int cap) { int g = grid_for(n, bloc
 template <bool FROM_BONDS>
 int launch_label_front(sw_handle* h, const Params& p, const uint8_t* bonds, int32_t* labels, cudaStream_t s)
 {
-    uint8_t* seamE = h->d_seam;
-    uint8_t* seamN = h->d_seam + (size_t)p.ntx * p.L;
     prof_mark(h, 0, s);
     k_scan<FROM_BONDS><<<dim3((p.ntx + SCAN_WARPS - 1) / SCAN_WARPS, p.nty), SCAN_THREADS, 0, s>>>(
-        p, h->d_spins, bonds, labels, seamE, seamN, h->d_acc);
+        p, h->d_spins, bonds, labels, h->d_edgeA, h->d_edgeB, h->d_acc);
     SW_LAUNCHED(h, "k_scan");
     prof_mark(h, 1, s);
     const int nseam = (p.ntx + p.nty) * p.L;
-    k_seam<<<grid_for(nseam, 256), 256, 0, s>>>(p, h->d_seam, labels);
+    k_seam<<<grid_for(nseam, 256), 256, 0, s>>>(p, h->d_edgeA, h->d_edgeB, labels);
     SW_LAUNCHED(h, "k_seam");
     prof_mark(h, 2, s);
     return SW_OK;
@@ -238,11 +238,12 @@ int sw_bind(sw_handle* h, void* d_spins, int32_t* d_labels, uint8_t* d_bonds, vo
     h->d_work = (uint8_t*)d_work;
     h->d_acc = (Acc*)(h->d_work + w.acc);
     h->d_wolff = (unsigned long long*)(h->d_work + w.wolff);
-    h->d_seam = h->d_work + w.seam;
+    h->d_edgeA = (int32_t*)(h->d_work + w.edgeA);
+    h->d_edgeB = (int32_t*)(h->d_work + w.edgeB);
     h->d_size = (int32_t*)(h->d_work + w.size);
     h->bound = false;
     h->have_labels = false;
-    SW_CUDA(h, cudaMemsetAsync(h->d_work, 0, w.seam, (cudaStream_t)stream));
+    SW_CUDA(h, cudaMemsetAsync(h->d_work, 0, w.edgeA, (cudaStream_t)stream));
     h->bound = true;
     return SW_OK;
 }
