@@ -34,8 +34,8 @@ __device__ __forceinline__ int strip_gidx(int base, int L, int l) { return base 
 // of any other site = the name (node) it adopted, so a chase that starts at any site ends at the root of its tree.
 // Private to one warp.
 //
-// find with path halving.  Roots change only through the atomicCAS in unite_batch; halving rewrites non-root entries
-// with an ancestor (plain store: concurrent lanes may interleave, every value written is an ancestor).
+// find with path halving.  Plain loads/stores: halving rewrites non-root entries with an ancestor (concurrent lanes may
+// interleave, every value written is an ancestor); roots change only in phase 2 of unite_batch.
 __device__ __forceinline__ int nm_find(volatile uint16_t* nm, int x)
 {
     int p = nm[x];
@@ -49,29 +49,36 @@ __device__ __forceinline__ int nm_find(volatile uint16_t* nm, int x)
     return x;
 }
 
-__device__ __forceinline__ int nm_root(const volatile uint16_t* nm, int x)
+// roots of four sites in lockstep (four independent chases per iteration)
+__device__ __forceinline__ void nm_root4(const volatile uint16_t* nm, int& a, int& b, int& c, int& d)
 {
-    int p = nm[x];
-    while (p != x) { x = p; p = nm[x]; }
-    return x;
+    int pa = nm[a], pb = nm[b], pc = nm[c], pd = nm[d];
+    while ((pa ^ a) | (pb ^ b) | (pc ^ c) | (pd ^ d)) {
+        a = pa; b = pb; c = pc; d = pd;
+        pa = nm[a]; pb = nm[b]; pc = nm[c]; pd = nm[d];
+    }
 }
 
-// Unite one queued pair of names per lane (pair = a << 16 | b): hook the larger root under the smaller with a 16-bit
-// compare-and-swap (it succeeds only while the larger one still is a root; otherwise retry from the new roots) and
-// write the hook through to `prov`.
+// Unite one queued pair of names per lane (pair = a << 16 | b), hooking the larger root under the smaller and writing
+// every hook through to `prov`.  3-phase protocol, no atomics (the forest belongs to this warp): (1) all lanes find
+// roots -- nobody hooks, so a root stays a root; (2) hook with a plain store -- lanes hooking the same root collide, one
+// store wins; (3) re-read: losers retry from the new roots.
 __device__ __forceinline__ void unite_batch(volatile uint16_t* nm, bool have, uint32_t pair, int* prov, int base, int L)
 {
     int ua = (int)(pair >> 16), ub = (int)(pair & 0xFFFFu);
-    while (have) {
-        ua = nm_find(nm, ua);
-        ub = nm_find(nm, ub);
-        if (ua == ub) break;
-        if (ua < ub) { const int t = ua; ua = ub; ub = t; }
-        const unsigned short old = atomicCAS(const_cast<unsigned short*>(reinterpret_cast<volatile unsigned short*>(nm)) + ua,
-                                             (unsigned short)ua, (unsigned short)ub);
-        if (old == (unsigned short)ua) {
+    while (__any_sync(FULLM, have)) {
+        if (have) {
+            ua = nm_find(nm, ua);
+            ub = nm_find(nm, ub);
+            if (ua == ub) have = false;
+            else if (ua < ub) { const int t = ua; ua = ub; ub = t; }
+        }
+        __syncwarp();
+        if (have) nm[ua] = (uint16_t)ub;
+        __syncwarp();
+        if (have && nm[ua] == ub) {
             prov[strip_gidx(base, L, ua)] = REF | HOOK | ub;
-            break;
+            have = false;
         }
     }
 }
@@ -286,25 +293,29 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
         if (colv) {
             // first row -> rootS, last row -> rootN (-1 where the north bond that leaves the strip is not active)
             const int lb0 = 4 * lane, lb1 = (th_eff - 1) * TW + 4 * lane;
+            int s0 = lb0, s1 = lb0 + 1, s2 = lb0 + 2, s3 = lb0 + 3;
+            int n0 = lb1, n1 = lb1 + 1, n2 = lb1 + 2, n3 = lb1 + 3;
+            nm_root4(vnm, s0, s1, s2, s3);
+            nm_root4(vnm, n0, n1, n2, n3);
             int4 s, n;
-            s.x = strip_gidx(base, L, nm_root(vnm, lb0));
-            s.y = strip_gidx(base, L, nm_root(vnm, lb0 + 1));
-            s.z = strip_gidx(base, L, nm_root(vnm, lb0 + 2));
-            s.w = strip_gidx(base, L, nm_root(vnm, lb0 + 3));
-            n.x = (northm & 1u) ? strip_gidx(base, L, nm_root(vnm, lb1)) : -1;
-            n.y = (northm & 2u) ? strip_gidx(base, L, nm_root(vnm, lb1 + 1)) : -1;
-            n.z = (northm & 4u) ? strip_gidx(base, L, nm_root(vnm, lb1 + 2)) : -1;
-            n.w = (northm & 8u) ? strip_gidx(base, L, nm_root(vnm, lb1 + 3)) : -1;
+            s.x = strip_gidx(base, L, s0);
+            s.y = strip_gidx(base, L, s1);
+            s.z = strip_gidx(base, L, s2);
+            s.w = strip_gidx(base, L, s3);
+            n.x = (northm & 1u) ? strip_gidx(base, L, n0) : -1;
+            n.y = (northm & 2u) ? strip_gidx(base, L, n1) : -1;
+            n.z = (northm & 4u) ? strip_gidx(base, L, n2) : -1;
+            n.w = (northm & 8u) ? strip_gidx(base, L, n3) : -1;
             *reinterpret_cast<int4*>(edgeB + (size_t)nE + (size_t)ty * L + x) = s;
             *reinterpret_cast<int4*>(edgeA + (size_t)nE + (size_t)ty * L + x) = n;
         }
         // first column -> rootW, last column -> rootE: lane i takes row i
         const uint32_t em = __shfl_sync(FULLM, eastm, last_lane);
         if (lane < th_eff) {
-            const int w = strip_gidx(base, L, nm_root(vnm, lane * TW));
-            const int e = ((em >> lane) & 1u) ? strip_gidx(base, L, nm_root(vnm, lane * TW + tw_eff - 1)) : -1;
-            edgeB[(size_t)tx * L + y0 + lane] = w;
-            edgeA[(size_t)tx * L + y0 + lane] = e;
+            int w = lane * TW, e = lane * TW + tw_eff - 1, w2 = w, e2 = e;
+            nm_root4(vnm, w, e, w2, e2);
+            edgeB[(size_t)tx * L + y0 + lane] = strip_gidx(base, L, w);
+            edgeA[(size_t)tx * L + y0 + lane] = ((em >> lane) & 1u) ? strip_gidx(base, L, e) : -1;
         }
     }
 
@@ -538,11 +549,13 @@ k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __rest
             uint32_t st[4];
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
-                int l = lb + j, w = ww[j];
-                if (w < 0) { l = w & LMASK; w = sm.S[l]; }
-                if (w < 0) { l = w & LMASK; w = sm.S[l]; }
-                ww[j] = w;
-                st[j] = MODE == MODE_SW ? sm.st[l] : 0u;
+                // own entry -> node -> strip-local root, as unconditional loads (a root / node just reads itself again)
+                const int w = ww[j];
+                const int i0 = w < 0 ? (w & LMASK) : lb + j;
+                const int w1 = sm.S[i0];
+                const int i1 = w1 < 0 ? (w1 & LMASK) : i0;
+                ww[j] = sm.S[i1];
+                st[j] = MODE == MODE_SW ? sm.st[i1] : 0u;
             }
             *reinterpret_cast<int4*>(labels + (size_t)y * L + x) = make_int4(ww[0], ww[1], ww[2], ww[3]);
             if (MODE == MODE_SW) {
