@@ -38,7 +38,7 @@ extern "C" {
 
 enum {
     SW_OK      = 0,
-    SW_EINVAL  = -1,  /* bad argument: L<4, L%4!=0, L>32768, q outside [2,8], beta not finite or <0, NULL or
+    SW_EINVAL  = -1,  /* bad argument: L<4, L%4!=0, L>32768 (L>16384 for q>2), q outside [2,8], beta not finite or <0, NULL or
                          misaligned pointer, workspace too small, n<0                                      */
     SW_ESTATE  = -2,  /* handle not bound (sw_bind not called), or d_bonds needed but bound as NULL        */
     SW_ECUDA   = -3,  /* a CUDA runtime call or kernel launch failed; text via sw_strerror / sw_last_cuda_error */
@@ -72,12 +72,12 @@ typedef struct {
 /* Create a handle for an L x L lattice of q-state spins at inverse temperature beta with RNG seed `seed`
  * (BASELINE.json north_star "sw_create(L,q,beta,seed)").  The bond threshold is T = floor((1-exp(-K beta)) 2^32)
  * in IEEE double on the host, K = 2 for q=2, K = 1 otherwise (S:8c.4); a bond between equal spins is activated
- * iff its 32-bit draw is < T (P:53 step 1, Eq. 7).  Requires 4 <= L <= 32768, L % 4 == 0, 2 <= q <= 8,
- * beta finite and >= 0.  The step counter starts at 0.  No device memory is allocated. */
+ * iff its 32-bit draw is < T (P:53 step 1, Eq. 7).  Requires 4 <= L <= 32768 (L <= 16384 if q > 2), L % 4 == 0,
+ * 2 <= q <= 8, beta finite and >= 0.  The step counter starts at 0.  No device memory is allocated. */
 int sw_create(sw_handle** out, int32_t L, int32_t q, double beta, uint64_t seed);
 int sw_destroy(sw_handle* h);
 
-/* Bytes of device workspace sw_bind needs for an L x L lattice (seam bond bytes, int32 cluster-size scratch,
+/* Bytes of device workspace sw_bind needs for an L x L lattice (int32 strip-edge root arrays, int32 cluster-size scratch,
  * accumulators).  0 if L or q is invalid. */
 size_t sw_workspace_bytes(int32_t L, int32_t q);
 

@@ -12,9 +12,15 @@ namespace swb {
 constexpr int TW_LOG = 7, TH_LOG = 5;
 constexpr int TW = 1 << TW_LOG;
 constexpr int TH = 1 << TH_LOG;
-constexpr int SCAN_WARPS = 4;                            // strips per k_scan CTA (horizontally adjacent)
+#ifndef SWB_SCAN_WARPS
+#define SWB_SCAN_WARPS 4
+#endif
+#ifndef SWB_FIN_THREADS
+#define SWB_FIN_THREADS 256
+#endif
+constexpr int SCAN_WARPS = SWB_SCAN_WARPS;               // strips per k_scan CTA (horizontally adjacent)
 constexpr int SCAN_THREADS = 32 * SCAN_WARPS;
-constexpr int FIN_THREADS = 256;
+constexpr int FIN_THREADS = SWB_FIN_THREADS;
 constexpr int FIN_WARPS = FIN_THREADS / 32;
 static_assert(TW == 128, "lane -> 4 columns, 32 lanes");
 static_assert(TW * TH <= 65536, "strip-local indices are kept in uint16");
@@ -27,6 +33,7 @@ struct Params {
     int32_t  L;          // edge length, multiple of 4
     int32_t  N;          // L*L <= 2^30
     int32_t  logL;       // log2(L) if L is a power of two, else -1
+    int32_t  sbit;       // k_final keeps a cluster's new state above this bit of its label: 28 if N <= 2^28, else 30
     int32_t  q;          // number of Potts states (2 = Ising storage +-1)
     int32_t  ntx, nty;   // number of tile columns / rows
     uint32_t T;          // bond threshold floor(p 2^32)

@@ -416,12 +416,11 @@ __device__ __forceinline__ uint32_t flip_state(const Params& p, int root)
     return __umulhi(w0, (uint32_t)p.q);                  // uniform state in [0,q)  (S:8c.6)
 }
 
-// Shared memory of k_final: the strip's entries (node entries are rewritten in place), one state byte per strip-local
-// root, and the compacted lists: strip-local roots from the front, hooked nodes from the back (together <= TW*TH).
+// Shared memory of k_final: the strip's entries (node entries are rewritten in place; a final root entry carries the
+// cluster's new state above bit Params::sbit) and the compacted lists: strip-local roots from the front, hooked nodes from the back (together <= TW*TH).
 struct FinalSmem {
     int      S[TW * TH];
     uint16_t list[TW * TH];
-    uint8_t  st[TW * TH];
     int      nroot, nhook;
     int      r0;
 };
@@ -437,7 +436,7 @@ struct FinalSmem {
 // then refers to it directly (concurrent rewrites only shorten paths).  (4) every site reaches its strip-local root in
 // at most two hops: own entry -> node -> root.
 template <int MODE>
-__global__ void __launch_bounds__(FIN_THREADS, 7)
+__global__ void __launch_bounds__(FIN_THREADS, 2048 / FIN_THREADS)
 k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __restrict__ acc,
         unsigned long long* __restrict__ wolff_size)
 {
@@ -518,12 +517,10 @@ k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __rest
             const int l = sm.list[k];
             int v = sm.S[l];
             const int g = strip_gidx(base, L, l);
-            if (v != g) {                                // hooked by k_seam: find the root of the global tree
-                v = gfind(labels, v);
-                sm.S[l] = v;
-            }
+            if (v != g) v = gfind(labels, v);            // hooked by k_seam: find the root of the global tree
             nroots += (v == g);
-            if (MODE == MODE_SW) sm.st[l] = (uint8_t)flip_state(p, v);
+            // final label and, above bit p.sbit, the new state of the cluster (labels are < 2^sbit)
+            sm.S[l] = MODE == MODE_SW ? (int)((uint32_t)v | (flip_state(p, v) << p.sbit)) : v;
         }
         const int nh = sm.nhook;
         volatile int* S = sm.S;
@@ -538,6 +535,7 @@ k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __rest
 
     // (4) every site
     const int r0 = MODE == MODE_WOLFF ? sm.r0 : -1;
+    const int lmask = (1 << p.sbit) - 1;
     int nflip = 0;
 #pragma unroll
     for (int r = 0; r < R; ++r) {
@@ -554,8 +552,9 @@ k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __rest
                 const int i0 = w < 0 ? (w & LMASK) : lb + j;
                 const int w1 = sm.S[i0];
                 const int i1 = w1 < 0 ? (w1 & LMASK) : i0;
-                ww[j] = sm.S[i1];
-                st[j] = MODE == MODE_SW ? sm.st[i1] : 0u;
+                const int w2 = sm.S[i1];
+                ww[j] = MODE == MODE_SW ? (w2 & lmask) : w2;
+                st[j] = MODE == MODE_SW ? (uint32_t)w2 >> p.sbit : 0u;
             }
             *reinterpret_cast<int4*>(labels + (size_t)y * L + x) = make_int4(ww[0], ww[1], ww[2], ww[3]);
             if (MODE == MODE_SW) {

@@ -63,7 +63,11 @@ WorkLayout work_layout(int32_t L)
     return w;
 }
 
-bool valid_shape(int32_t L, int32_t q) { return L >= 4 && L <= 32768 && (L % 4) == 0 && q >= 2 && q <= 8; }
+// labels are < N <= 2^30; k_final packs the new state (q <= 8: 3 bits) above the label, which needs N <= 2^28 unless q = 2
+bool valid_shape(int32_t L, int32_t q)
+{
+    return L >= 4 && L <= 32768 && (L % 4) == 0 && q >= 2 && q <= 8 && (q == 2 || L <= 16384);
+}
 
 int cuda_fail(sw_handle* h, cudaError_t e, const char* where)
 {
@@ -166,6 +170,7 @@ int sw_create(sw_handle** out, int32_t L, int32_t q, double beta, uint64_t seed)
     Params& p = h->p;
     p.L = L; p.N = (int32_t)h->N; p.q = q;
     p.logL = -1;
+    p.sbit = h->N <= (1 << 28) ? 28 : 30;
     for (int k = 2; k <= 15; ++k) if ((1 << k) == L) p.logL = k;
     p.ntx = (L + TW - 1) / TW; p.nty = (L + TH - 1) / TH;
     const uint32_t s_lo = (uint32_t)(seed & 0xFFFFFFFFu), s_hi = (uint32_t)(seed >> 32);
