@@ -400,9 +400,11 @@ k_seam(const Params p, const int* __restrict__ edgeA, const int* __restrict__ ed
             rb = edgeB[idb];
         }
     }
-    // the previous seam site joins the same two strip-local clusters: skip (its thread does the union)
-    const int pa = __shfl_up_sync(FULLM, ra, 1), pb = __shfl_up_sync(FULLM, rb, 1);
-    const bool dup = (threadIdx.x & 31) != 0 && pa == ra && pb == rb;
+    // the previous ACTIVE seam site of this warp joins the same two strip-local clusters: skip (its thread does the union)
+    const unsigned act = __ballot_sync(FULLM, ra >= 0);
+    const int prev = 31 - __clz(act & lanemask_lt());    // -1: none
+    const int pa = __shfl_sync(FULLM, ra, prev & 31), pb = __shfl_sync(FULLM, rb, prev & 31);
+    const bool dup = prev >= 0 && pa == ra && pb == rb;
     if (ra >= 0 && !dup) gunite(prov, ra, rb);
 }
 
@@ -474,10 +476,10 @@ k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __rest
             if (y < L && colv) {
                 const int4 v = *reinterpret_cast<const int4*>(labels + (size_t)y * L + x);
                 *reinterpret_cast<int4*>(&sm.S[ly * TW + 4 * lane]) = v;
-                rootm |= ((v.x >= 0) | ((v.y >= 0) << 1) | ((v.z >= 0) << 2) | ((v.w >= 0) << 3)) << (4 * r);
-                constexpr int RH = REF | HOOK;
-                hookm |= (((v.x & RH) == RH) | (((v.y & RH) == RH) << 1) | (((v.z & RH) == RH) << 2) |
-                          (((v.w & RH) == RH) << 3)) << (4 * r);
+                // top bytes of the 4 entries; bit 7 clear: root, bits 7 and 6 set: hooked node; 4 spread bits -> 4 adjacent
+                const uint32_t t = __byte_perm(__byte_perm(v.x, v.y, 0x0073), __byte_perm(v.z, v.w, 0x0073), 0x5410);
+                rootm |= (((~t & 0x80808080u) * 0x00204081u) >> 28) << (4 * r);
+                hookm |= (((t & (t << 1) & 0x80808080u) * 0x00204081u) >> 28) << (4 * r);
             }
         }
         const int cnt = __popc(rootm) | (__popc(hookm) << 16);
