@@ -343,19 +343,6 @@ __device__ __forceinline__ int strip_root(const int* prov, int L, int site, int 
 // only ever changes to a smaller index of the same (growing) set, so a stale read is still an ancestor.  Path halving
 // writes an ancestor with a plain store; it can race with the atomicMin of a retrying hook, which then still unites
 // the displaced parent.
-__device__ __forceinline__ int gfind_halve(int* prov, int x)
-{
-    int pp = __ldcg(prov + x);
-    while (pp != x) {
-        const int gp = __ldcg(prov + pp);
-        if (gp == pp) return pp;
-        prov[x] = gp;
-        x = gp;
-        pp = __ldcg(prov + x);
-    }
-    return x;
-}
-
 __device__ __forceinline__ int gfind(const int* prov, int x)
 {
     int pp = __ldcg(prov + x);
@@ -363,11 +350,21 @@ __device__ __forceinline__ int gfind(const int* prov, int x)
     return x;
 }
 
+// Unite the trees of a and b.  Both finds advance in lockstep (two independent loads per round trip), with path halving:
+// one round trip when both are roots already, two when each is one hop from its root.
 __device__ __forceinline__ void gunite(int* prov, int a, int b)
 {
     while (true) {
-        a = gfind_halve(prov, a);
-        b = gfind_halve(prov, b);
+        while (true) {
+            const int pa = __ldcg(prov + a), pb = __ldcg(prov + b);
+            if (pa == a && pb == b) break;
+            const int ga = __ldcg(prov + pa), gb = __ldcg(prov + pb);
+            if (pa != a && ga != pa) prov[a] = ga;       // path halving
+            if (pb != b && gb != pb) prov[b] = gb;
+            const bool done = ga == pa && gb == pb;      // both parents are roots
+            a = ga; b = gb;
+            if (done) break;
+        }
         if (a == b) return;
         if (a < b) { const int t = a; a = b; b = t; }    // a > b: hook a under b
         const int old = atomicMin(prov + a, b);
@@ -377,7 +374,8 @@ __device__ __forceinline__ void gunite(int* prov, int a, int b)
 }
 
 // One thread per seam site (ids [0, ntx*L): east seams (strip column tc, row y); then nty*L north seams (strip row tr,
-// column x)): if its crossing bond is active (edgeA >= 0), unite the strip-local roots of its two ends.
+// column x)): if its crossing bond is active (edgeA >= 0), unite the strip-local roots of its two ends.  Both edge
+// entries are loaded up front (the index of the facing entry does not depend on the first load).
 __global__ void __launch_bounds__(256)
 k_seam(const Params p, const int* __restrict__ edgeA, const int* __restrict__ edgeB, int* prov)
 {
@@ -386,19 +384,16 @@ k_seam(const Params p, const int* __restrict__ edgeA, const int* __restrict__ ed
     const int id = blockIdx.x * blockDim.x + threadIdx.x;
     int ra = -1, rb = -1;
     if (id < nseam) {
-        ra = edgeA[id];
-        if (ra >= 0) {
-            int idb;
-            if (id < nE) {                               // first column of the strip column to the east (periodic)
-                const int tc = div_L(p, (uint32_t)id);
-                idb = tc + 1 == p.ntx ? id - tc * L : id + L;
-            } else {                                     // first row of the strip row to the north (periodic)
-                const int k = id - nE;
-                const int tr = div_L(p, (uint32_t)k);
-                idb = tr + 1 == p.nty ? id - tr * L : id + L;
-            }
-            rb = edgeB[idb];
+        int idb;
+        if (id < nE) {                                   // first column of the strip column to the east (periodic)
+            const int tc = div_L(p, (uint32_t)id);
+            idb = tc + 1 == p.ntx ? id - tc * L : id + L;
+        } else {                                         // first row of the strip row to the north (periodic)
+            const int tr = div_L(p, (uint32_t)(id - nE));
+            idb = tr + 1 == p.nty ? id - tr * L : id + L;
         }
+        ra = edgeA[id];
+        rb = edgeB[idb];
     }
     // the previous ACTIVE seam site of this warp joins the same two strip-local clusters: skip (its thread does the union)
     const unsigned act = __ballot_sync(FULLM, ra >= 0);
@@ -418,12 +413,13 @@ __device__ __forceinline__ uint32_t flip_state(const Params& p, int root)
     return __umulhi(w0, (uint32_t)p.q);                  // uniform state in [0,q)  (S:8c.6)
 }
 
-// Shared memory of k_final: the strip's entries (node entries are rewritten in place; a final root entry carries the
-// cluster's new state above bit Params::sbit) and the compacted lists: strip-local roots from the front, hooked nodes from the back (together <= TW*TH).
+// Shared memory of k_final: the strip's entries (node entries are rewritten in place with the FINAL value of their
+// cluster: the canonical label and, in MODE_SW, the cluster's new state above bit Params::sbit -- a value >= 0) and the
+// compacted list of the strip-local roots.
 struct FinalSmem {
     int      S[TW * TH];
     uint16_t list[TW * TH];
-    int      nroot, nhook;
+    int      nroot;
     int      r0;
 };
 
@@ -431,12 +427,13 @@ struct FinalSmem {
 //   MODE_SW    : s_i = state drawn for the root (assign, P:55 step 3)
 //   MODE_WOLFF : s_i = -s_i iff root(i) == root(seed site i0); adds |C| to *wolff_size
 //   MODE_LABEL : labels only
-// (1) the strip's entries go to shared memory; roots and hooked nodes are compacted into lists.  (2) every strip-local
+// (1) the strip's entries go to shared memory; the strip-local roots are compacted into a list.  (2) every strip-local
 // root is resolved to the root of its global tree (a chase over entries >= 0 of other strips, which concurrently running
 // CTAs may already have overwritten with final labels -- those are roots of the same tree, so the chase still ends at the
-// right root) and draws one Philox state.  (3) every hooked node follows its references to the strip-local root and
-// then refers to it directly (concurrent rewrites only shorten paths).  (4) every site reaches its strip-local root in
-// at most two hops: own entry -> node -> root.
+// right root) and draws one Philox state; its entry becomes the final value.  (3) every hooked node (each thread looks
+// after its own sites) follows its references to the first entry >= 0 -- the strip-local root or a hooked node that is
+// final already, both carry the final value of the cluster -- and takes that value.  (4) every other site is one hop
+// from a node.
 template <int MODE>
 __global__ void __launch_bounds__(FIN_THREADS, 2048 / FIN_THREADS)
 k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __restrict__ acc,
@@ -452,10 +449,10 @@ k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __rest
     const bool colv = 4 * lane < tw_eff;
     const int ly0 = warp * R;
     const int base = y0 * L + x0;
+    volatile int* S = sm.S;
 
     if (threadIdx.x == 0) {
         sm.nroot = 0;
-        sm.nhook = 0;
         if (MODE == MODE_WOLFF) {
             uint32_t w0, w1, w2, w3;
             philox4x32_10(p, 0u, p.t_lo, p.t_hi, DOM_WSEED, w0, w1, w2, w3);
@@ -465,11 +462,12 @@ k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __rest
             sm.r0 = gfind(labels, strip_root(labels, L, i0, b0));
         }
     }
-    __syncthreads();                                     // counters (and r0) visible
+    __syncthreads();                                     // counter (and r0) visible
 
-    // (1) entries -> shared memory; compact roots (from the front of sm.list) and hooked nodes (from the back)
+    // (1) entries -> shared memory; compact the roots into sm.list
+    uint32_t hookm = 0;                                  // bit 4r+j: my site (row r, column j) is a hooked node
     {
-        uint32_t rootm = 0, hookm = 0;                   // bit 4r+j: my site (row r, column j) is a root / a hooked node
+        uint32_t rootm = 0;                              // ... is a strip-local root
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const int ly = ly0 + r, y = y0 + ly;
@@ -482,36 +480,24 @@ k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __rest
                 hookm |= (((t & (t << 1) & 0x80808080u) * 0x00204081u) >> 28) << (4 * r);
             }
         }
-        const int cnt = __popc(rootm) | (__popc(hookm) << 16);
+        const int cnt = __popc(rootm);
         int incl = cnt;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
             const int t = __shfl_up_sync(FULLM, incl, o);
             if (lane >= o) incl += t;
         }
-        int rbase = 0, hbase = 0;
-        if (lane == 31) {
-            if (incl & 0xFFFF) rbase = atomicAdd(&sm.nroot, incl & 0xFFFF);
-            if (incl >> 16) hbase = atomicAdd(&sm.nhook, incl >> 16);
-        }
+        int rbase = 0;
+        if (lane == 31 && incl) rbase = atomicAdd(&sm.nroot, incl);
         rbase = __shfl_sync(FULLM, rbase, 31);
-        hbase = __shfl_sync(FULLM, hbase, 31);
-        const int excl = incl - cnt;
-        int pos = rbase + (excl & 0xFFFF);
+        int pos = rbase + incl - cnt;
         for (uint32_t m = rootm; m; m &= m - 1) {
             const int b = __ffs(m) - 1;
             sm.list[pos++] = (uint16_t)((ly0 + (b >> 2)) * TW + 4 * lane + (b & 3));
         }
-        pos = TW * TH - 1 - (hbase + (excl >> 16));
-        for (uint32_t m = hookm; m; m &= m - 1) {
-            const int b = __ffs(m) - 1;
-            sm.list[pos--] = (uint16_t)((ly0 + (b >> 2)) * TW + 4 * lane + (b & 3));
-        }
     }
     __syncthreads();
-    // (2) one global resolve + one Philox draw per strip-local root, (3) one chase per hooked node; both balanced over
-    // the CTA.  (3) only reads and writes references (< 0), (2) only root entries (>= 0), so they need no barrier
-    // between them.
+    // (2) one global resolve + one Philox draw per strip-local root, balanced over the CTA
     int nroots = 0;
     {
         const int n = sm.nroot;
@@ -524,14 +510,15 @@ k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __rest
             // final label and, above bit p.sbit, the new state of the cluster (labels are < 2^sbit)
             sm.S[l] = MODE == MODE_SW ? (int)((uint32_t)v | (flip_state(p, v) << p.sbit)) : v;
         }
-        const int nh = sm.nhook;
-        volatile int* S = sm.S;
-        for (int k = threadIdx.x; k < nh; k += FIN_THREADS) {
-            const int l = sm.list[TW * TH - 1 - k];
-            int r = S[l] & LMASK, e = S[r];
-            while (e < 0) { r = e & LMASK; e = S[r]; }
-            S[l] = REF | r;
-        }
+    }
+    __syncthreads();
+    // (3) my hooked nodes
+    for (uint32_t m = hookm; m; m &= m - 1) {
+        const int b = __ffs(m) - 1;
+        const int l = (ly0 + (b >> 2)) * TW + 4 * lane + (b & 3);
+        int e = S[l];
+        do { e = S[e & LMASK]; } while (e < 0);
+        S[l] = e;
     }
     __syncthreads();
 
@@ -543,20 +530,15 @@ k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __rest
     for (int r = 0; r < R; ++r) {
         const int ly = ly0 + r, y = y0 + ly;
         if (y < L && colv) {
-            const int lb = ly * TW + 4 * lane;
-            const int4 v = *reinterpret_cast<const int4*>(&sm.S[lb]);
+            const int4 v = *reinterpret_cast<const int4*>(&sm.S[ly * TW + 4 * lane]);
             int ww[4] = {v.x, v.y, v.z, v.w};
             uint32_t st[4];
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
-                // own entry -> node -> strip-local root, as unconditional loads (a root / node just reads itself again)
-                const int w = ww[j];
-                const int i0 = w < 0 ? (w & LMASK) : lb + j;
-                const int w1 = sm.S[i0];
-                const int i1 = w1 < 0 ? (w1 & LMASK) : i0;
-                const int w2 = sm.S[i1];
-                ww[j] = MODE == MODE_SW ? (w2 & lmask) : w2;
-                st[j] = MODE == MODE_SW ? (uint32_t)w2 >> p.sbit : 0u;
+                int w = ww[j];
+                if (w < 0) w = sm.S[w & LMASK];          // not a node: one hop to its node, which is final
+                ww[j] = MODE == MODE_SW ? (w & lmask) : w;
+                st[j] = MODE == MODE_SW ? (uint32_t)w >> p.sbit : 0u;
             }
             *reinterpret_cast<int4*>(labels + (size_t)y * L + x) = make_int4(ww[0], ww[1], ww[2], ww[3]);
             if (MODE == MODE_SW) {
