@@ -91,240 +91,11 @@ constexpr int QCAP = 32 + TW;                            // < 32 pairs carried o
 //           (east bond of the last column, north bond of the last row) is not active
 //   edgeB = [ rootW (ntx * L) | rootS (nty * L) ] : first column / first row, same indexing
 //
-// One warp per TW x TH strip, lane -> 4 consecutive columns, rows in sequence.  FROM_BONDS=false: read spins, draw
-// bonds (a1).  FROM_BONDS=true: read packed bonds (sw_label).  Writes the provisional labels described above and the
-// edge arrays, and adds the number of active bonds to acc->n_active.
-//
-// Row step.  A "node" is a horizontal run (inside the strip) that has no active north bond from the row above; it is
-// named by its first site.  Every other run adopts the name carried by its leftmost contact with the row above, so
-// every name is a node.  When a run has further contacts whose names differ from the adopted one, the pair of names is
-// queued; queued pairs are united 32 at a time (all lanes busy) in the strip's forest.  Names never depend on the
-// forest, so the row loop has no divergent part.
-template <bool FROM_BONDS>
-__global__ void __launch_bounds__(SCAN_THREADS)
-k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __restrict__ bonds_in, int* prov,
-       int* __restrict__ edgeA, int* __restrict__ edgeB, Acc* __restrict__ acc)
-{
-    __shared__ __align__(16) uint16_t s_nm[SCAN_WARPS][TW * TH];
-    __shared__ uint32_t s_q[SCAN_WARPS][QCAP];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int tx = blockIdx.x * SCAN_WARPS + warp, ty = blockIdx.y;
-    if (tx >= p.ntx) return;                             // no block-wide barrier in this kernel
-    uint16_t* nm = s_nm[warp];
-    volatile uint16_t* vnm = nm;
-    volatile uint32_t* q = s_q[warp];
-    const int L = p.L, Lw = L >> 2;
-    const int x0 = tx * TW, y0 = ty * TH;
-    const int tw_eff = min(TW, L - x0), th_eff = min(TH, L - y0);
-    const int x = x0 + 4 * lane;
-    const bool colv = 4 * lane < tw_eff;
-    const int last_lane = (tw_eff >> 2) - 1;             // lane that owns the strip's last column
-    const bool is_last = lane == last_lane;
-    const int base = y0 * L + x0;
-    const int xw = x >> 2;
-    const int xew = ((x + 4 == L) ? 0 : x + 4) >> 2;     // east halo word of the last lane (periodic)
-    const unsigned lt = lanemask_lt(), me = 1u << lane, le = lt | me, gt = ~le;
+}  // namespace swb
 
-    // spin words of rows y, y+1, y+2 (w*) and the east halo words of the last lane (h*); row index L wraps to 0
-    uint32_t w0 = 0, w1 = 0, w2 = 0, h0 = 0, h1 = 0, h2 = 0;
-    if (!FROM_BONDS) {
-        const int yend = y0 + th_eff;                    // north neighbour row of the strip's last row
-        if (colv) {
-            w0 = spins_w[(size_t)y0 * Lw + xw];
-            if (is_last) h0 = spins_w[(size_t)y0 * Lw + xew];
-            const int ya = y0 + 1, yb = y0 + 2;
-            if (ya <= yend) { const int yy = ya == L ? 0 : ya; w1 = spins_w[(size_t)yy * Lw + xw]; if (is_last) h1 = spins_w[(size_t)yy * Lw + xew]; }
-            if (yb <= yend) { const int yy = yb == L ? 0 : yb; w2 = spins_w[(size_t)yy * Lw + xw]; if (is_last) h2 = spins_w[(size_t)yy * Lw + xew]; }
-        }
-    }
+#include "scan_kernel.cuh"
 
-    int Lp0 = NONE, Lp1 = NONE, Lp2 = NONE, Lp3 = NONE;  // names carried by the previous row's sites
-    uint32_t np = 0;                                     // active north bonds from the previous row into this row
-    int nact = 0;
-    int qn = 0;                                          // queued pairs (warp-uniform)
-    uint32_t eastm = 0;                                  // last lane: bit ly = the east bond that leaves the strip in row ly
-    uint32_t northm = 0;                                 // the 4 north bonds that leave the strip in the last row
-
-    for (int ly = 0; ly < th_eff; ++ly) {
-        const int y = y0 + ly;
-        uint32_t e4 = 0, n4 = 0;
-        if (!FROM_BONDS) {
-            uint32_t w3 = 0, h3 = 0;                     // prefetch row y+3
-            {
-                const int yc = y + 3;
-                if (colv && yc <= y0 + th_eff) {
-                    const int yy = yc == L ? 0 : yc;
-                    w3 = spins_w[(size_t)yy * Lw + xw];
-                    if (is_last) h3 = spins_w[(size_t)yy * Lw + xew];
-                }
-            }
-            uint32_t wnext = __shfl_down_sync(FULLM, w0, 1);
-            if (is_last) wnext = h0;
-            if (colv) {
-                const uint32_t east = __funnelshift_r(w0, wnext, 8);
-                const uint32_t eqe = eq_bytes4(w0, east);
-                const uint32_t eqn = eq_bytes4(w0, w1);
-                const uint32_t c0 = (uint32_t)(y * L + x) >> 1;
-                uint32_t a0, a1, a2, a3, b0, b1, b2, b3;
-                philox4x32_10(p, c0, p.t_lo, p.t_hi, DOM_BOND, a0, a1, a2, a3);
-                philox4x32_10(p, c0 + 1, p.t_lo, p.t_hi, DOM_BOND, b0, b1, b2, b3);
-                const uint32_t de = (a0 < p.T) | ((a2 < p.T) << 1) | ((b0 < p.T) << 2) | ((b2 < p.T) << 3);
-                const uint32_t dn = (a1 < p.T) | ((a3 < p.T) << 1) | ((b1 < p.T) << 2) | ((b3 < p.T) << 3);
-                e4 = eqe & de;
-                n4 = eqn & dn;
-                nact += __popc(e4) + __popc(n4);
-            }
-            w0 = w1; w1 = w2; w2 = w3; h0 = h1; h1 = h2; h2 = h3;
-        } else if (colv) {
-            const uint32_t b = bonds_in[((size_t)y * L + x) >> 2];
-            e4 = (b & 1) | ((b >> 1) & 2) | ((b >> 2) & 4) | ((b >> 3) & 8);
-            n4 = ((b >> 1) & 1) | ((b >> 2) & 2) | ((b >> 3) & 4) | ((b >> 4) & 8);
-        }
-
-        // bonds that leave the strip are remembered for the edge arrays and dropped here
-        if (is_last) {
-            eastm |= (e4 >> 3) << ly;
-            e4 &= 7u;
-        }
-        if (ly == th_eff - 1) {
-            northm = n4;
-            n4 = 0;
-        }
-
-        // ---- names of this row's sites ----------------------------------------------------------------------
-        const bool E0 = e4 & 1u, E1 = e4 & 2u, E2 = e4 & 4u, E3 = e4 & 8u;
-        const bool full = (e4 & 7u) == 7u;
-        const bool EL = (__shfl_up_sync(FULLM, e4, 1) & 8u) && lane;
-        const int ref0 = REF | (ly * TW + 4 * lane);
-        // leftmost contact of every intra-lane segment: forward pass, then spread back from the segment end
-        const int c0 = (np & 1u) ? Lp0 : NONE, c1 = (np & 2u) ? Lp1 : NONE;
-        const int c2 = (np & 4u) ? Lp2 : NONE, c3 = (np & 8u) ? Lp3 : NONE;
-        const int f1 = (E0 && c0 < 0) ? c0 : c1;
-        const int f2 = (E1 && f1 < 0) ? f1 : c2;
-        const int f3 = (E2 && f2 < 0) ? f2 : c3;
-        const int g2 = E2 ? f3 : f2;
-        const int g1 = E1 ? g2 : f1;
-        const int g0 = E0 ? g1 : c0;
-        const int s1 = E0 ? 0 : 1, s2 = E1 ? s1 : 2, s3 = E2 ? s2 : 3;      // first site of each site's segment
-        const int pubP = g0;                                                // my prefix segment: contact or NONE
-        const int pubS = f3 < 0 ? f3 : ref0 + s3;                           // my suffix segment: contact or new node
-
-        // runs that cross lane boundaries: lanes a..b, a's suffix segment, full lanes, b's prefix segment
-        const unsigned LINK = __ballot_sync(FULLM, E3);
-        const unsigned FULLB = __ballot_sync(FULLM, full);
-        const unsigned CS = __ballot_sync(FULLM, f3 < 0);
-        const unsigned CP = __ballot_sync(FULLM, g0 < 0);
-        const unsigned nPTL = ~(FULLB & (LINK << 1));                       // lanes where a run cannot pass to the left
-        const unsigned nPTR = ~(FULLB & LINK);                              // ... to the right
-        const int a_le = 31 - __clz(nPTL & le);                             // bit 0 of nPTL is always set
-        const int a_lt = 31 - __clz(nPTL & lt);                             // -1 on lane 0 (unused there: EL = 0)
-        const int bS = E3 ? __ffs(nPTR & gt) - 1 : lane;                    // bit 31 of nPTR is always set
-        const unsigned MS = (CS & ((1u << bS) - 1u) & (FULLM << a_le)) | (CP & (1u << bS));
-        const int srcS = MS ? __ffs(MS) - 1 : a_le;
-        const unsigned MP = (CS & lt & (FULLM << (a_lt & 31))) | (CP & me);
-        const int srcP = MP ? __ffs(MP) - 1 : a_lt;
-        const int vS1 = __shfl_sync(FULLM, pubS, srcS & 31);
-        const int vP1 = __shfl_sync(FULLM, pubP, bS);
-        const int vS2 = __shfl_sync(FULLM, pubS, srcP & 31);
-        const int RS = (srcS == bS) ? vP1 : vS1;                            // name of the run my suffix segment is in
-        const int RP = (srcP == lane) ? g0 : vS2;                           // ... my prefix segment (if not full)
-        const bool useS = E3 || (full && EL), useP = EL && !full;
-
-        int l0 = g0 < 0 ? g0 : ref0;
-        int l1 = g1 < 0 ? g1 : ref0 + s1;
-        int l2 = g2 < 0 ? g2 : ref0 + s2;
-        int l3 = f3 < 0 ? f3 : ref0 + s3;
-        if (useP) { l0 = RP; if (s1 == 0) l1 = RP; if (s2 == 0) l2 = RP; }
-        if (useS) { l3 = RS; if (s2 == s3) l2 = RS; if (s1 == s3) l1 = RS; if (s3 == 0) l0 = RS; }
-
-        // the row's entries in the forest (a new node's name is its own index, i.e. it starts as a root) and in `prov`
-        if (colv) {
-            uint2 o;
-            o.x = ((uint32_t)l0 & 0xFFFFu) | ((uint32_t)l1 << 16);
-            o.y = ((uint32_t)l2 & 0xFFFFu) | ((uint32_t)l3 << 16);
-            *reinterpret_cast<uint2*>(nm + ly * TW + 4 * lane) = o;
-            const int gi = y * L + x;
-            int4 g;
-            g.x = l0 == ref0 ? gi : l0;
-            g.y = l1 == ref0 + 1 ? gi + 1 : l1;
-            g.z = l2 == ref0 + 2 ? gi + 2 : l2;
-            g.w = l3 == ref0 + 3 ? gi + 3 : l3;
-            *reinterpret_cast<int4*>(prov + (size_t)gi) = g;
-        }
-
-        // contacts whose carried name differs from the adopted one: queue the pair of names
-        {
-            const bool m0 = (np & 1u) && Lp0 != l0, m1 = (np & 2u) && Lp1 != l1;
-            const bool m2 = (np & 4u) && Lp2 != l2, m3 = (np & 8u) && Lp3 != l3;
-            const unsigned B0 = __ballot_sync(FULLM, m0), B1 = __ballot_sync(FULLM, m1);
-            const unsigned B2 = __ballot_sync(FULLM, m2), B3 = __ballot_sync(FULLM, m3);
-            if (m0) q[qn + __popc(B0 & lt)] = __byte_perm((uint32_t)l0, (uint32_t)Lp0, 0x5410);
-            qn += __popc(B0);
-            if (m1) q[qn + __popc(B1 & lt)] = __byte_perm((uint32_t)l1, (uint32_t)Lp1, 0x5410);
-            qn += __popc(B1);
-            if (m2) q[qn + __popc(B2 & lt)] = __byte_perm((uint32_t)l2, (uint32_t)Lp2, 0x5410);
-            qn += __popc(B2);
-            if (m3) q[qn + __popc(B3 & lt)] = __byte_perm((uint32_t)l3, (uint32_t)Lp3, 0x5410);
-            qn += __popc(B3);
-        }
-        if (qn >= 32) {
-            __syncwarp();                                // queue, forest entries and `prov` rows visible to the whole warp
-            do {
-                qn -= 32;
-                unite_batch(vnm, true, q[qn + lane], prov, base, L);
-            } while (qn >= 32);
-            __syncwarp();                                // queue slots read before the next row overwrites them
-        }
-
-        Lp0 = l0; Lp1 = l1; Lp2 = l2; Lp3 = l3;
-        np = n4;
-    }
-
-    __syncwarp();
-    if (qn > 0) {
-        const bool have = lane < qn;
-        unite_batch(vnm, have, have ? q[lane] : 0u, prov, base, L);
-    }
-    __syncwarp();
-
-    // ---- edge arrays: strip-local roots of the sites on the four edges ----------------------------------------------
-    {
-        const int nE = p.ntx * L;
-        if (colv) {
-            // first row -> rootS, last row -> rootN (-1 where the north bond that leaves the strip is not active)
-            const int lb0 = 4 * lane, lb1 = (th_eff - 1) * TW + 4 * lane;
-            int s0 = lb0, s1 = lb0 + 1, s2 = lb0 + 2, s3 = lb0 + 3;
-            int n0 = lb1, n1 = lb1 + 1, n2 = lb1 + 2, n3 = lb1 + 3;
-            nm_root4(vnm, s0, s1, s2, s3);
-            nm_root4(vnm, n0, n1, n2, n3);
-            int4 s, n;
-            s.x = strip_gidx(base, L, s0);
-            s.y = strip_gidx(base, L, s1);
-            s.z = strip_gidx(base, L, s2);
-            s.w = strip_gidx(base, L, s3);
-            n.x = (northm & 1u) ? strip_gidx(base, L, n0) : -1;
-            n.y = (northm & 2u) ? strip_gidx(base, L, n1) : -1;
-            n.z = (northm & 4u) ? strip_gidx(base, L, n2) : -1;
-            n.w = (northm & 8u) ? strip_gidx(base, L, n3) : -1;
-            *reinterpret_cast<int4*>(edgeB + (size_t)nE + (size_t)ty * L + x) = s;
-            *reinterpret_cast<int4*>(edgeA + (size_t)nE + (size_t)ty * L + x) = n;
-        }
-        // first column -> rootW, last column -> rootE: lane i takes row i
-        const uint32_t em = __shfl_sync(FULLM, eastm, last_lane);
-        if (lane < th_eff) {
-            int w = lane * TW, e = lane * TW + tw_eff - 1, w2 = w, e2 = e;
-            nm_root4(vnm, w, e, w2, e2);
-            edgeB[(size_t)tx * L + y0 + lane] = strip_gidx(base, L, w);
-            edgeA[(size_t)tx * L + y0 + lane] = ((em >> lane) & 1u) ? strip_gidx(base, L, e) : -1;
-        }
-    }
-
-    if (!FROM_BONDS) {
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) nact += __shfl_xor_sync(FULLM, nact, o);
-        if (lane == 0 && nact) atomicAdd(&acc->n_active, (unsigned long long)nact);
-    }
-}
+namespace swb {
 
 // ------------------------------------------------------------------------------------------------ seams
 // strip-local root (global index) of `site`: follow the strip-local references

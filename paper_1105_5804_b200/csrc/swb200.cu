@@ -102,6 +102,7 @@ Params params_at(const sw_handle* h, uint64_t t)
 {
     Params p = h->p;
     p.T = h->T;
+    p.negT = 4294967296ull - (uint64_t)h->T;
     p.t_lo = (uint32_t)(t & 0xFFFFFFFFu);
     p.t_hi = (uint32_t)(t >> 32);
     return p;
@@ -121,8 +122,11 @@ template <bool FROM_BONDS>
 int launch_label_front(sw_handle* h, const Params& p, const uint8_t* bonds, int32_t* labels, cudaStream_t s)
 {
     prof_mark(h, 0, s);
-    k_scan<FROM_BONDS><<<dim3((p.ntx + SCAN_WARPS - 1) / SCAN_WARPS, p.nty), SCAN_THREADS, 0, s>>>(
-        p, h->d_spins, bonds, labels, h->d_edgeA, h->d_edgeB, h->d_acc);
+    const dim3 grid((p.ntx + SCAN_WARPS - 1) / SCAN_WARPS, p.nty);
+    if (FROM_BONDS || p.q == 2)
+        k_scan<FROM_BONDS, true><<<grid, SCAN_THREADS, 0, s>>>(p, h->d_spins, bonds, labels, h->d_edgeA, h->d_edgeB, h->d_acc);
+    else
+        k_scan<false, false><<<grid, SCAN_THREADS, 0, s>>>(p, h->d_spins, bonds, labels, h->d_edgeA, h->d_edgeB, h->d_acc);
     SW_LAUNCHED(h, "k_scan");
     prof_mark(h, 1, s);
     const int nseam = (p.ntx + p.nty) * p.L;
@@ -177,6 +181,11 @@ int sw_create(sw_handle** out, int32_t L, int32_t q, double beta, uint64_t seed)
     for (int r = 0; r < 10; ++r) {
         p.k0[r] = s_lo + (uint32_t)r * 0x9E3779B9u;
         p.k1[r] = s_hi + (uint32_t)r * 0xBB67AE85u;
+    }
+    p.one = 1u;
+    for (int j = 0; j < 4; ++j) {
+        p.wt[2 * j] = 1u << (8 * j + 1);
+        p.wt[2 * j + 1] = 1u << (8 * j + 2);
     }
     *out = h;
     return SW_OK;
