@@ -40,10 +40,8 @@ struct Params {
     uint32_t t_lo, t_hi; // step counter
     uint32_t k0[10];     // Philox round keys: k0[r] = seed_lo + r * 0x9E3779B9
     uint32_t k1[10];     //                    k1[r] = seed_hi + r * 0xBB67AE85
-    // k_scan's draw-to-bit arithmetic on the multiply-add pipe (scan_kernel.cuh acc_ge): values the compiler must not fold
-    uint32_t one;        // 1
-    uint32_t wt[8];      // bit weights of the 8 draws of a lane's row: 2^(8j+1) east, 2^(8j+2) north, site j = 0..3
-    uint64_t negT;       // 2^32 - T
+    uint32_t negT;       // 2^32 - T (mod 2^32): u + negT carries iff u >= T, for T != 0 (scan_kernel.cuh shift_in_ge)
+    uint32_t dmask;      // 0xFF; 0 if T = 0 (no bond is ever active)
 };
 
 // Philox4x32-10 (Salmon et al., SC'11).  c1,c2,c3 are warp-uniform in every use here (step counter and domain).

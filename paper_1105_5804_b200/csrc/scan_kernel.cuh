@@ -85,18 +85,20 @@ constexpr ScanLut make_scan_lut()
 __device__ const ScanLut d_scan_lut = make_scan_lut();
 
 // ---------------------------------------------------------------------------------------------------- helpers
-__device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t s) { return __byte_perm(a, b, s); }
-
-// [u >= T] as the carry of u + (2^32 - T), accumulated at a bit position: acc + carry * weight.  Two multiply-adds
-// (the FMA pipe) instead of a compare, a select and a shift-or on the ALU pipe, which is the one that saturates.
-__device__ __forceinline__ uint32_t acc_ge(uint32_t acc, uint32_t u, uint32_t one, uint64_t negT, uint32_t weight)
+// PRMT reads the 4 selector nibbles of s[15:0] only (every nibble here is < 8: plain byte select); __byte_perm would
+// spend an extra instruction masking the selector.
+__device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t s)
 {
-    uint32_t hi;
-    asm("{\n\t.reg .u64 t;\n\t.reg .u32 lo;\n\tmad.wide.u32 t, %1, %2, %3;\n\tmov.b64 {lo, %0}, t;\n\t}"
-        : "=r"(hi) : "r"(u), "r"(one), "l"(negT));
-    uint32_t r;
-    asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(r) : "r"(hi), "r"(weight), "r"(acc));
-    return r;
+    uint32_t d;
+    asm("prmt.b32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(s));
+    return d;
+}
+
+// d <- 2 d + [u >= T] for T != 0: the carry of u + (2^32 - T) shifted into d.  An add with carry-out (ALU pipe) and an
+// add with carry-in (ptxas issues it as IMAD.X on the multiply-add pipe): no compare, select or shift.
+__device__ __forceinline__ void shift_in_ge(uint32_t& d, uint32_t u, uint32_t negT)
+{
+    asm("{\n\t.reg .u32 t;\n\tadd.cc.u32 t, %1, %2;\n\taddc.u32 %0, %0, %0;\n\t}" : "+r"(d) : "r"(u), "r"(negT));
 }
 
 // The lane's bond byte for row y: bit 2j = east bond of site j, bit 2j+1 = north bond of site j (the packed-bond
@@ -107,26 +109,20 @@ __device__ __forceinline__ uint32_t bond_byte(const Params& p, uint32_t c0, uint
     uint32_t a0, a1, a2, a3, b0, b1, b2, b3;
     philox4x32_10(p, c0, p.t_lo, p.t_hi, DOM_BOND, a0, a1, a2, a3);
     philox4x32_10(p, c0 + 1, p.t_lo, p.t_hi, DOM_BOND, b0, b1, b2, b3);
-    // d: bit 8j+1 = [east draw of site j >= T], bit 8j+2 = [north draw >= T]
+    // d: bit 2j = [east draw of site j >= T], bit 2j+1 = [north draw >= T]: the last draw first, it ends up in bit 7
     uint32_t d = 0;
-    d = acc_ge(d, a0, p.one, p.negT, p.wt[0]);
-    d = acc_ge(d, a1, p.one, p.negT, p.wt[1]);
-    d = acc_ge(d, a2, p.one, p.negT, p.wt[2]);
-    d = acc_ge(d, a3, p.one, p.negT, p.wt[3]);
-    d = acc_ge(d, b0, p.one, p.negT, p.wt[4]);
-    d = acc_ge(d, b1, p.one, p.negT, p.wt[5]);
-    d = acc_ge(d, b2, p.one, p.negT, p.wt[6]);
-    d = acc_ge(d, b3, p.one, p.negT, p.wt[7]);
+    shift_in_ge(d, b3, p.negT); shift_in_ge(d, b2, p.negT); shift_in_ge(d, b1, p.negT); shift_in_ge(d, b0, p.negT);
+    shift_in_ge(d, a3, p.negT); shift_in_ge(d, a2, p.negT); shift_in_ge(d, a1, p.negT); shift_in_ge(d, a0, p.negT);
     uint32_t eq;                                         // bit 8j+1: s_j == s_east, bit 8j+2: s_j == s_north
     if (ISING) {                                         // bytes 0x01 / 0xFF: equal <=> bit 1 (and bit 2) of the xor is 0
         eq = (~(w ^ e) & 0x02020202u) | (~(w ^ n) & 0x04040404u);
     } else {
         eq = (__vcmpeq4(w, e) & 0x02020202u) | (__vcmpeq4(w, n) & 0x04040404u);
     }
-    const uint32_t b = eq & ~d;
     // gather the 4 bit pairs (8j+1, 8j+2) into bits (2j, 2j+1) of the high word; the cross terms of the product land on
     // distinct bits below 32 or above bit 7 of the high word (no carries)
-    return __umulhi(b, 0x82082000u) & 0xFFu;             // 2^31 + 2^25 + 2^19 + 2^13
+    // p.dmask = 0xFF, or 0 if T = 0 (then u >= T always, but u + 2^32 never carries)
+    return __umulhi(eq, 0x82082000u) & ~d & p.dmask;     // 2^31 + 2^25 + 2^19 + 2^13
 }
 
 // ---------------------------------------------------------------------------------------------------- k_scan
@@ -163,21 +159,23 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
     const int xw = x >> 2;
     const int xew = ((x + 4 == L) ? 0 : x + 4) >> 2;     // east halo word of the last lane (periodic)
     const unsigned lt = lanemask_lt(), me = 1u << lane, le = lt | me, gt = ~le;
-    const uint32_t gmask = is_last ? 0xBFu : 0xFFu;      // the east bond that leaves the strip is dropped from the byte
+    // the east bond that leaves the strip is dropped from the lane's bond byte; lanes beyond a ragged edge have no bonds
+    const uint32_t gmask = !colv ? 0u : is_last ? 0xBFu : 0xFFu;
 
     // spin words of rows y, y+1, y+2 (w*) and the east halo words of the last lane (h*); row index L wraps to 0
     uint32_t w0 = 0, w1 = 0, w2 = 0, h0 = 0, h1 = 0, h2 = 0;
     const int yend = y0 + th_eff;                        // north neighbour row of the strip's last row
     const int row_halo = (yend == L ? 0 : yend) * Lw;    // its word offset
-    if (!FROM_BONDS && colv) {
-        w0 = spins_w[(size_t)y0 * Lw + xw];
+    const int xws = colv ? xw : (x0 >> 2);               // lanes beyond a ragged edge read a valid word (their bonds are masked)
+    if (!FROM_BONDS) {
+        w0 = spins_w[(size_t)y0 * Lw + xws];
         if (is_last) h0 = spins_w[(size_t)y0 * Lw + xew];
         const int r1 = th_eff > 1 ? (y0 + 1) * Lw : row_halo;
-        w1 = spins_w[r1 + xw];
+        w1 = spins_w[r1 + xws];
         if (is_last) h1 = spins_w[r1 + xew];
         if (th_eff > 1) {
             const int r2 = th_eff > 2 ? (y0 + 2) * Lw : row_halo;
-            w2 = spins_w[r2 + xw];
+            w2 = spins_w[r2 + xws];
             if (is_last) h2 = spins_w[r2 + xew];
         }
     }
@@ -190,37 +188,40 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
     int nlink = 0;                                       // active east bonds between lanes (warp-uniform)
     int qn = 0;                                          // queued pairs (warp-uniform)
     uint32_t eastm = 0;                                  // last lane: bit (th_eff-1-ly) = the east bond that leaves the strip
-    uint32_t northm = 0;                                 // the 4 north bonds that leave the strip in the last row (bits 1,3,5,7)
+    uint32_t northm = 0;                                 // bond byte of the last row: its north bonds (bits 1,3,5,7) leave the strip
+
+    // running per-row quantities: word offset of the row to prefetch (ly + 3), Philox counter of the lane's first pair,
+    // global index of the lane's first site
+    int ro = (y0 + 3) * Lw;
+    uint32_t c0 = (uint32_t)(y0 * L + x) >> 1;
+    int gi = y0 * L + x;
+    const uint32_t* const pw = spins_w + xws;            // the lane's word column / its east halo column
+    const uint32_t* const ph = spins_w + xew;
 
     for (int ly = 0; ly < th_eff; ++ly) {
-        const int y = y0 + ly;
         uint32_t G = 0;                                  // the lane's bond byte of this row
         if (!FROM_BONDS) {
-            uint32_t w3 = 0, h3 = 0;                     // prefetch row y+3
-            {
-                const int r = ly + 3;
-                if (r <= th_eff && colv) {
-                    const int ro = r < th_eff ? (y + 3) * Lw : row_halo;
-                    w3 = spins_w[ro + xw];
-                    if (is_last) h3 = spins_w[ro + xew];
-                }
+            uint32_t w3 = 0, h3 = 0;                     // prefetch row y+3 (the last one is the north halo row)
+            if (ly + 3 <= th_eff) {
+                const int o = ly + 3 < th_eff ? ro : row_halo;
+                w3 = pw[o];
+                if (is_last) h3 = ph[o];
             }
+            ro += Lw;
             uint32_t wnext = __shfl_down_sync(FULLM, w0, 1);
             if (is_last) wnext = h0;
             const uint32_t east = __funnelshift_r(w0, wnext, 8);
-            G = bond_byte<ISING>(p, (uint32_t)(y * L + x) >> 1, w0, east, w1);
-            if (!colv) G = 0;
+            G = bond_byte<ISING>(p, c0, w0, east, w1);
+            c0 += (uint32_t)L >> 1;
             w0 = w1; w1 = w2; w2 = w3; h0 = h1; h1 = h2; h2 = h3;
         } else if (colv) {
-            G = bonds_in[((size_t)y * L + x) >> 2];
+            G = bonds_in[(size_t)gi >> 2];
         }
         // bonds that leave the strip are remembered for the edge arrays and dropped here
+        // (the north bonds of the last row are not used inside the loop: they only feed the next row's table index)
         eastm = eastm * 2u + ((G >> 6) & 1u);
         G &= gmask;
-        if (ly == th_eff - 1) {
-            northm = G & 0xAAu;
-            G &= 0x55u;
-        }
+        northm = G;
 
         // ---- names of this row's sites ----------------------------------------------------------------------
         const uint32_t EL = (__shfl_up_sync(FULLM, G, 1) >> 5) & (lane ? 2u : 0u);
@@ -236,8 +237,8 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
         const bool E3 = G & 0x40u;
         const unsigned LINK = __ballot_sync(FULLM, E3);
         const unsigned FULLB = __ballot_sync(FULLM, (G & 0x15u) == 0x15u);
-        const unsigned CS = __ballot_sync(FULLM, A.w & 1u);
-        const unsigned CP = __ballot_sync(FULLM, A.w & 2u);
+        const unsigned CS = __ballot_sync(FULLM, (A.w & 1u) != 0u);
+        const unsigned CP = __ballot_sync(FULLM, (A.w & 2u) != 0u);
         nlink += __popc(LINK);
         const unsigned nPTL = ~(FULLB & (LINK << 1));                       // lanes where a run cannot pass to the left
         const unsigned nPTR = ~(FULLB & LINK);                              // ... to the right
@@ -255,7 +256,6 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
         // the row's entries in the forest (a new node's name is its own index, i.e. it starts as a root) and in `prov`
         *reinterpret_cast<uint2*>(nm + ly * TW + 4 * lane) = make_uint2(l01, l23);
         if (colv) {
-            const int gi = y * L + x;
             const uint32_t z01 = l01 ^ NEW01, z23 = l23 ^ NEW23;
             int4 g;
             g.x = (z01 & 0xFFFFu) ? (int)prmt(l01, 0x80000000u, 0x7610) : gi;
@@ -294,8 +294,10 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
         npm = G & 0xAAu;
         NEW01 += (uint32_t)TW * 0x00010001u;
         NEW23 += (uint32_t)TW * 0x00010001u;
+        gi += L;
     }
 
+    northm &= 0xAAu;
     __syncwarp();
     if (qn > 0) {
         const bool have = lane < qn;

@@ -102,7 +102,8 @@ Params params_at(const sw_handle* h, uint64_t t)
 {
     Params p = h->p;
     p.T = h->T;
-    p.negT = 4294967296ull - (uint64_t)h->T;
+    p.negT = 0u - h->T;
+    p.dmask = h->T ? 0xFFu : 0u;
     p.t_lo = (uint32_t)(t & 0xFFFFFFFFu);
     p.t_hi = (uint32_t)(t >> 32);
     return p;
@@ -181,11 +182,6 @@ int sw_create(sw_handle** out, int32_t L, int32_t q, double beta, uint64_t seed)
     for (int r = 0; r < 10; ++r) {
         p.k0[r] = s_lo + (uint32_t)r * 0x9E3779B9u;
         p.k1[r] = s_hi + (uint32_t)r * 0xBB67AE85u;
-    }
-    p.one = 1u;
-    for (int j = 0; j < 4; ++j) {
-        p.wt[2 * j] = 1u << (8 * j + 1);
-        p.wt[2 * j + 1] = 1u << (8 * j + 2);
     }
     *out = h;
     return SW_OK;
