@@ -121,40 +121,38 @@ __device__ __forceinline__ int gfind(const int* prov, int x)
     return x;
 }
 
-// Unite the trees of a and b.  Both finds advance in lockstep (two independent loads per round trip), with path halving:
-// one round trip when both are roots already, two when each is one hop from its root.
-__device__ __forceinline__ void gunite(int* prov, int a, int b)
+// Unite the trees of a and b; pa, pb = entries of a and b, loaded by the caller.  Both finds advance in lockstep (two
+// independent loads per round trip), with path halving: nothing more to load when both are roots already, one round
+// trip when each is one hop from its root.
+__device__ __forceinline__ void gunite(int* prov, int a, int b, int pa, int pb)
 {
     while (true) {
-        while (true) {
-            const int pa = __ldcg(prov + a), pb = __ldcg(prov + b);
-            if (pa == a && pb == b) break;
+        while (pa != a || pb != b) {
             const int ga = __ldcg(prov + pa), gb = __ldcg(prov + pb);
             if (pa != a && ga != pa) prov[a] = ga;       // path halving
             if (pb != b && gb != pb) prov[b] = gb;
             const bool done = ga == pa && gb == pb;      // both parents are roots
             a = ga; b = gb;
             if (done) break;
+            pa = __ldcg(prov + a); pb = __ldcg(prov + b);
         }
         if (a == b) return;
         if (a < b) { const int t = a; a = b; b = t; }    // a > b: hook a under b
         const int old = atomicMin(prov + a, b);
         if (old == a) return;                            // a was a root and now points to b
         a = old;                                         // a had been hooked meanwhile: entry = min(old,b); join old and b
+        pa = __ldcg(prov + a); pb = __ldcg(prov + b);
     }
 }
 
-// One thread per seam site (ids [0, ntx*L): east seams (strip column tc, row y); then nty*L north seams (strip row tr,
-// column x)): if its crossing bond is active (edgeA >= 0), unite the strip-local roots of its two ends.  Both edge
-// entries are loaded up front (the index of the facing entry does not depend on the first load).
-__global__ void __launch_bounds__(256)
-k_seam(const Params p, const int* __restrict__ edgeA, const int* __restrict__ edgeB, int* prov)
+// Seam site `id` (ids [0, ntx*L): east seams (strip column tc, row y); then nty*L north seams (strip row tr, column x)):
+// the strip-local roots of its two ends, ra = -1 if its crossing bond is not active.
+__device__ __forceinline__ void seam_ends(const Params& p, const int* __restrict__ edgeA, const int* __restrict__ edgeB,
+                                          int id, int nE, int nseam, int& ra, int& rb)
 {
-    const int L = p.L;
-    const int nE = p.ntx * L, nseam = (p.ntx + p.nty) * L;
-    const int id = blockIdx.x * blockDim.x + threadIdx.x;
-    int ra = -1, rb = -1;
+    ra = -1; rb = -1;
     if (id < nseam) {
+        const int L = p.L;
         int idb;
         if (id < nE) {                                   // first column of the strip column to the east (periodic)
             const int tc = div_L(p, (uint32_t)id);
@@ -166,12 +164,35 @@ k_seam(const Params p, const int* __restrict__ edgeA, const int* __restrict__ ed
         ra = edgeA[id];
         rb = edgeB[idb];
     }
-    // the previous ACTIVE seam site of this warp joins the same two strip-local clusters: skip (its thread does the union)
+}
+
+// true if this lane has a union to do: its bond is active and the previous ACTIVE seam site of the warp does not join the
+// same two strip-local clusters (then that lane does the union)
+__device__ __forceinline__ bool seam_todo(int ra, int rb)
+{
     const unsigned act = __ballot_sync(FULLM, ra >= 0);
     const int prev = 31 - __clz(act & lanemask_lt());    // -1: none
     const int pa = __shfl_sync(FULLM, ra, prev & 31), pb = __shfl_sync(FULLM, rb, prev & 31);
-    const bool dup = prev >= 0 && pa == ra && pb == rb;
-    if (ra >= 0 && !dup) gunite(prov, ra, rb);
+    return ra >= 0 && !(prev >= 0 && pa == ra && pb == rb);
+}
+
+// Two seam sites per thread (id and id + half): all four edge entries are loaded up front, then the four root entries,
+// so that a thread has up to four independent loads in flight; then the two unions.
+__global__ void __launch_bounds__(256)
+k_seam(const Params p, const int* __restrict__ edgeA, const int* __restrict__ edgeB, int* prov)
+{
+    const int nE = p.ntx * p.L, nseam = (p.ntx + p.nty) * p.L;
+    const int half = ((nseam + 63) >> 6) << 5;           // multiple of 32: a warp's ids stay consecutive
+    const int id = blockIdx.x * blockDim.x + threadIdx.x;
+    int ra0, rb0, ra1, rb1;
+    seam_ends(p, edgeA, edgeB, id < half ? id : nseam, nE, nseam, ra0, rb0);
+    seam_ends(p, edgeA, edgeB, id < half ? id + half : nseam, nE, nseam, ra1, rb1);
+    const bool t0 = seam_todo(ra0, rb0), t1 = seam_todo(ra1, rb1);
+    int pa0 = 0, pb0 = 0, pa1 = 0, pb1 = 0;
+    if (t0) { pa0 = __ldcg(prov + ra0); pb0 = __ldcg(prov + rb0); }
+    if (t1) { pa1 = __ldcg(prov + ra1); pb1 = __ldcg(prov + rb1); }
+    if (t0) gunite(prov, ra0, rb0, pa0, pb0);
+    if (t1) gunite(prov, ra1, rb1, pa1, pb1);
 }
 
 // ------------------------------------------------------------------------------------------------ k_final
@@ -185,26 +206,32 @@ __device__ __forceinline__ uint32_t flip_state(const Params& p, int root)
 }
 
 // Shared memory of k_final: the strip's entries (node entries are rewritten in place with the FINAL value of their
-// cluster: the canonical label and, in MODE_SW, the cluster's new state above bit Params::sbit -- a value >= 0) and the
-// compacted list of the strip-local roots.
+// cluster: the canonical label and, in MODE_SW, the cluster's new state above bit Params::sbit -- a value >= 0) and, per
+// warp, the list of the strip-local roots among the warp's own rows.
 struct FinalSmem {
     int      S[TW * TH];
     uint16_t list[TW * TH];
-    int      nroot;
     int      r0;
 };
+
+__device__ __forceinline__ int lds_s32(uint32_t saddr)
+{
+    int v;
+    asm volatile("ld.shared.s32 %0, [%1];" : "=r"(v) : "r"(saddr));
+    return v;
+}
 
 // One CTA per strip: canonical labels (root of every site) + the new spins.
 //   MODE_SW    : s_i = state drawn for the root (assign, P:55 step 3)
 //   MODE_WOLFF : s_i = -s_i iff root(i) == root(seed site i0); adds |C| to *wolff_size
 //   MODE_LABEL : labels only
-// (1) the strip's entries go to shared memory; the strip-local roots are compacted into a list.  (2) every strip-local
-// root is resolved to the root of its global tree (a chase over entries >= 0 of other strips, which concurrently running
-// CTAs may already have overwritten with final labels -- those are roots of the same tree, so the chase still ends at the
-// right root) and draws one Philox state; its entry becomes the final value.  (3) every hooked node (each thread looks
-// after its own sites) follows its references to the first entry >= 0 -- the strip-local root or a hooked node that is
-// final already, both carry the final value of the cluster -- and takes that value.  (4) every other site is one hop
-// from a node.
+// (1) every warp copies its rows of entries to shared memory and lists the strip-local roots among them; (2) it resolves
+// each of them to the root of its global tree (a chase over entries >= 0 of other strips, which concurrently running CTAs
+// may already have overwritten with final labels -- those are roots of the same tree, so the chase still ends at the
+// right root) and draws one Philox state; the entry becomes the final value.  Up to here a warp touches its own rows
+// only: no block barrier.  (3) every hooked node (each thread looks after its own sites) follows its references to the
+// first entry >= 0 -- the strip-local root or a hooked node that is final already, both carry the final value of the
+// cluster -- and takes that value.  (4) every other site is one hop from a node.
 template <int MODE>
 __global__ void __launch_bounds__(FIN_THREADS, 2048 / FIN_THREADS)
 k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __restrict__ acc,
@@ -222,9 +249,8 @@ k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __rest
     const int base = y0 * L + x0;
     volatile int* S = sm.S;
 
-    if (threadIdx.x == 0) {
-        sm.nroot = 0;
-        if (MODE == MODE_WOLFF) {
+    if (MODE == MODE_WOLFF) {
+        if (threadIdx.x == 0) {
             uint32_t w0, w1, w2, w3;
             philox4x32_10(p, 0u, p.t_lo, p.t_hi, DOM_WSEED, w0, w1, w2, w3);
             const int i0 = (int)__umulhi(w0, (uint32_t)p.N);
@@ -233,10 +259,11 @@ k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __rest
             sm.r0 = gfind(labels, strip_root(labels, L, i0, b0));
         }
     }
-    __syncthreads();                                     // counter (and r0) visible
 
-    // (1) entries -> shared memory; compact the roots into sm.list
+    // (1) my warp's rows -> shared memory; its roots -> its part of sm.list
     uint32_t hookm = 0;                                  // bit 4r+j: my site (row r, column j) is a hooked node
+    uint16_t* const mylist = sm.list + warp * (R * TW);
+    int nmine;                                           // roots in my warp's rows
     {
         uint32_t rootm = 0;                              // ... is a strip-local root
 #pragma unroll
@@ -258,29 +285,24 @@ k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __rest
             const int t = __shfl_up_sync(FULLM, incl, o);
             if (lane >= o) incl += t;
         }
-        int rbase = 0;
-        if (lane == 31 && incl) rbase = atomicAdd(&sm.nroot, incl);
-        rbase = __shfl_sync(FULLM, rbase, 31);
-        int pos = rbase + incl - cnt;
+        nmine = __shfl_sync(FULLM, incl, 31);
+        int pos = incl - cnt;
         for (uint32_t m = rootm; m; m &= m - 1) {
             const int b = __ffs(m) - 1;
-            sm.list[pos++] = (uint16_t)((ly0 + (b >> 2)) * TW + 4 * lane + (b & 3));
+            mylist[pos++] = (uint16_t)((ly0 + (b >> 2)) * TW + 4 * lane + (b & 3));
         }
     }
-    __syncthreads();
-    // (2) one global resolve + one Philox draw per strip-local root, balanced over the CTA
+    __syncwarp();
+    // (2) one global resolve + one Philox draw per strip-local root, balanced over the warp
     int nroots = 0;
-    {
-        const int n = sm.nroot;
-        for (int k = threadIdx.x; k < n; k += FIN_THREADS) {
-            const int l = sm.list[k];
-            int v = sm.S[l];
-            const int g = strip_gidx(base, L, l);
-            if (v != g) v = gfind(labels, v);            // hooked by k_seam: find the root of the global tree
-            nroots += (v == g);
-            // final label and, above bit p.sbit, the new state of the cluster (labels are < 2^sbit)
-            sm.S[l] = MODE == MODE_SW ? (int)((uint32_t)v | (flip_state(p, v) << p.sbit)) : v;
-        }
+    for (int k = lane; k < nmine; k += 32) {
+        const int l = mylist[k];
+        int v = sm.S[l];
+        const int g = strip_gidx(base, L, l);
+        if (v != g) v = gfind(labels, v);                // hooked by k_seam: find the root of the global tree
+        nroots += (v == g);
+        // final label and, above bit p.sbit, the new state of the cluster (labels are < 2^sbit)
+        sm.S[l] = MODE == MODE_SW ? (int)((uint32_t)v | (flip_state(p, v) << p.sbit)) : v;
     }
     __syncthreads();
     // (3) my hooked nodes
@@ -296,27 +318,30 @@ k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __rest
     // (4) every site
     const int r0 = MODE == MODE_WOLFF ? sm.r0 : -1;
     const int lmask = (1 << p.sbit) - 1;
+    const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(sm.S);
+    const uint32_t sshift = (uint32_t)p.sbit - 24u, smask = 0x01010101u * ((1u << (31 - p.sbit)) - 1u);
     int nflip = 0;
+    int* lrow = labels + (size_t)(y0 + ly0) * L + x;
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         const int ly = ly0 + r, y = y0 + ly;
         if (y < L && colv) {
             const int4 v = *reinterpret_cast<const int4*>(&sm.S[ly * TW + 4 * lane]);
             int ww[4] = {v.x, v.y, v.z, v.w};
-            uint32_t st[4];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                int w = ww[j];
-                if (w < 0) w = sm.S[w & LMASK];          // not a node: one hop to its node, which is final
-                ww[j] = MODE == MODE_SW ? (w & lmask) : w;
-                st[j] = MODE == MODE_SW ? (uint32_t)w >> p.sbit : 0u;
-            }
-            *reinterpret_cast<int4*>(labels + (size_t)y * L + x) = make_int4(ww[0], ww[1], ww[2], ww[3]);
+            for (int j = 0; j < 4; ++j)                  // not a node: one hop to its node, which is final
+                if (ww[j] < 0) ww[j] = lds_s32(sbase + (((uint32_t)ww[j] << 2) & (uint32_t)(LMASK << 2)));
             if (MODE == MODE_SW) {
-                uint32_t word = st[0] | (st[1] << 8) | (st[2] << 16) | (st[3] << 24);
+                // the 4 top bytes hold the states above bit sbit - 24
+                const uint32_t t = __byte_perm(__byte_perm(ww[0], ww[1], 0x0073), __byte_perm(ww[2], ww[3], 0x0073), 0x5410);
+                uint32_t word = (t >> sshift) & smask;
                 if (p.q == 2) word = 0x01010101u | (word * 0xFEu);   // k=0 -> +1 (0x01), k=1 -> -1 (0xFF)
                 spins_w[((size_t)y * L + x) >> 2] = word;
-            } else if (MODE == MODE_WOLFF) {
+                *reinterpret_cast<int4*>(lrow) = make_int4(ww[0] & lmask, ww[1] & lmask, ww[2] & lmask, ww[3] & lmask);
+            } else {
+                *reinterpret_cast<int4*>(lrow) = make_int4(ww[0], ww[1], ww[2], ww[3]);
+            }
+            if (MODE == MODE_WOLFF) {
                 const uint32_t m = (ww[0] == r0 ? 0xFFu : 0u) | (ww[1] == r0 ? 0xFF00u : 0u) |
                                    (ww[2] == r0 ? 0xFF0000u : 0u) | (ww[3] == r0 ? 0xFF000000u : 0u);   // bytes to negate
                 if (m) {
@@ -326,6 +351,7 @@ k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __rest
                 }
             }
         }
+        lrow += L;
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
