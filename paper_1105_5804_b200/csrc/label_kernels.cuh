@@ -176,23 +176,37 @@ __device__ __forceinline__ bool seam_todo(int ra, int rb)
     return ra >= 0 && !(prev >= 0 && pa == ra && pb == rb);
 }
 
-// Two seam sites per thread (id and id + half): all four edge entries are loaded up front, then the four root entries,
-// so that a thread has up to four independent loads in flight; then the two unions.
+// SEAM_PER_THREAD seam sites per thread (id, id + part, ...): all edge entries are loaded up front, then all root
+// entries, so that a thread has many independent loads in flight (the kernel is bound by memory latency); then the unions.
+#ifndef SWB_SEAM_PER_THREAD
+#define SWB_SEAM_PER_THREAD 4
+#endif
+constexpr int SEAM_PER_THREAD = SWB_SEAM_PER_THREAD;
+__host__ __device__ inline int seam_part(int nseam)     // ids per part, a multiple of 32: a warp's ids stay consecutive
+{
+    return ((nseam + 32 * SEAM_PER_THREAD - 1) / (32 * SEAM_PER_THREAD)) * 32;
+}
+
 __global__ void __launch_bounds__(256)
 k_seam(const Params p, const int* __restrict__ edgeA, const int* __restrict__ edgeB, int* prov)
 {
     const int nE = p.ntx * p.L, nseam = (p.ntx + p.nty) * p.L;
-    const int half = ((nseam + 63) >> 6) << 5;           // multiple of 32: a warp's ids stay consecutive
+    const int part = seam_part(nseam);
     const int id = blockIdx.x * blockDim.x + threadIdx.x;
-    int ra0, rb0, ra1, rb1;
-    seam_ends(p, edgeA, edgeB, id < half ? id : nseam, nE, nseam, ra0, rb0);
-    seam_ends(p, edgeA, edgeB, id < half ? id + half : nseam, nE, nseam, ra1, rb1);
-    const bool t0 = seam_todo(ra0, rb0), t1 = seam_todo(ra1, rb1);
-    int pa0 = 0, pb0 = 0, pa1 = 0, pb1 = 0;
-    if (t0) { pa0 = __ldcg(prov + ra0); pb0 = __ldcg(prov + rb0); }
-    if (t1) { pa1 = __ldcg(prov + ra1); pb1 = __ldcg(prov + rb1); }
-    if (t0) gunite(prov, ra0, rb0, pa0, pb0);
-    if (t1) gunite(prov, ra1, rb1, pa1, pb1);
+    int ra[SEAM_PER_THREAD], rb[SEAM_PER_THREAD], pa[SEAM_PER_THREAD], pb[SEAM_PER_THREAD];
+    bool todo[SEAM_PER_THREAD];
+#pragma unroll
+    for (int k = 0; k < SEAM_PER_THREAD; ++k)
+        seam_ends(p, edgeA, edgeB, id < part ? id + k * part : nseam, nE, nseam, ra[k], rb[k]);
+#pragma unroll
+    for (int k = 0; k < SEAM_PER_THREAD; ++k) {
+        todo[k] = seam_todo(ra[k], rb[k]);
+        pa[k] = pb[k] = 0;
+        if (todo[k]) { pa[k] = __ldcg(prov + ra[k]); pb[k] = __ldcg(prov + rb[k]); }
+    }
+#pragma unroll
+    for (int k = 0; k < SEAM_PER_THREAD; ++k)
+        if (todo[k]) gunite(prov, ra[k], rb[k], pa[k], pb[k]);
 }
 
 // ------------------------------------------------------------------------------------------------ k_final

@@ -131,7 +131,7 @@ int launch_label_front(sw_handle* h, const Params& p, const uint8_t* bonds, int3
     SW_LAUNCHED(h, "k_scan");
     prof_mark(h, 1, s);
     const int nseam = (p.ntx + p.nty) * p.L;
-    k_seam<<<grid_for((((int64_t)nseam + 63) >> 6) << 5, 256), 256, 0, s>>>(p, h->d_edgeA, h->d_edgeB, labels);
+    k_seam<<<grid_for(seam_part(nseam), 256), 256, 0, s>>>(p, h->d_edgeA, h->d_edgeB, labels);
     SW_LAUNCHED(h, "k_seam");
     prof_mark(h, 2, s);
     return SW_OK;
