@@ -190,24 +190,24 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
     uint32_t eastm = 0;                                  // last lane: bit (th_eff-1-ly) = the east bond that leaves the strip
     uint32_t northm = 0;                                 // bond byte of the last row: its north bonds (bits 1,3,5,7) leave the strip
 
-    // running per-row quantities: word offset of the row to prefetch (ly + 3), Philox counter of the lane's first pair,
-    // global index of the lane's first site
-    int ro = (y0 + 3) * Lw;
+    // running per-row quantities: Philox counter of the lane's first pair, global index of the lane's first site, pointer
+    // to the lane's spin word of the row to prefetch (ly + 3)
     uint32_t c0 = (uint32_t)(y0 * L + x) >> 1;
     int gi = y0 * L + x;
-    const uint32_t* const pw = spins_w + xws;            // the lane's word column / its east halo column
-    const uint32_t* const ph = spins_w + xew;
+    const uint32_t* pw = spins_w + (size_t)(y0 + 3) * Lw + xws;   // the lane's word of the row to prefetch; halo: + dxe
+    const uint32_t* const pw_halo = spins_w + row_halo + xws;
+    const int dxe = xew - xws;
 
     for (int ly = 0; ly < th_eff; ++ly) {
         uint32_t G = 0;                                  // the lane's bond byte of this row
         if (!FROM_BONDS) {
             uint32_t w3 = 0, h3 = 0;                     // prefetch row y+3 (the last one is the north halo row)
             if (ly + 3 <= th_eff) {
-                const int o = ly + 3 < th_eff ? ro : row_halo;
-                w3 = pw[o];
-                if (is_last) h3 = ph[o];
+                const uint32_t* const q3 = ly + 3 < th_eff ? pw : pw_halo;
+                w3 = *q3;
+                if (is_last) h3 = q3[dxe];
             }
-            ro += Lw;
+            pw += Lw;
             uint32_t wnext = __shfl_down_sync(FULLM, w0, 1);
             if (is_last) wnext = h0;
             const uint32_t east = __funnelshift_r(w0, wnext, 8);
@@ -272,14 +272,16 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
             const bool m0 = d01 & 0xFFFFu, m1 = d01 >> 16, m2 = d23 & 0xFFFFu, m3 = d23 >> 16;
             const unsigned B0 = __ballot_sync(FULLM, m0), B1 = __ballot_sync(FULLM, m1);
             const unsigned B2 = __ballot_sync(FULLM, m2), B3 = __ballot_sync(FULLM, m3);
-            if (m0) q[qn + __popc(B0 & lt)] = prmt(l01, P01, 0x5410);
-            qn += __popc(B0);
-            if (m1) q[qn + __popc(B1 & lt)] = prmt(l01, P01, 0x7632);
-            qn += __popc(B1);
-            if (m2) q[qn + __popc(B2 & lt)] = prmt(l23, P23, 0x5410);
-            qn += __popc(B2);
-            if (m3) q[qn + __popc(B3 & lt)] = prmt(l23, P23, 0x7632);
-            qn += __popc(B3);
+            volatile uint32_t* qp = q + qn;
+            if (m0) qp[__popc(B0 & lt)] = prmt(l01, P01, 0x5410);
+            qp += __popc(B0);
+            if (m1) qp[__popc(B1 & lt)] = prmt(l01, P01, 0x7632);
+            qp += __popc(B1);
+            if (m2) qp[__popc(B2 & lt)] = prmt(l23, P23, 0x5410);
+            qp += __popc(B2);
+            if (m3) qp[__popc(B3 & lt)] = prmt(l23, P23, 0x7632);
+            qp += __popc(B3);
+            qn = (int)(qp - q);
         }
         if (qn >= 32) {
             __syncwarp();                                // queue, forest entries and `prov` rows visible to the whole warp
