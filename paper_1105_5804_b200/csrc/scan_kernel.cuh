@@ -23,8 +23,8 @@ constexpr uint32_t lut_half(int h) { return (uint32_t)(((2 * h + 1) << 4) | (2 *
 constexpr uint32_t lut_sel(int hlo, int hhi) { return lut_half(hlo) | (lut_half(hhi) << 8); }
 
 struct ScanLut {
-    uint32_t a[256][4];    // index = the lane's bond byte pattern: bits 0,2,4 = E0,E1,E2 (east bonds site j -> j+1 of this
-                           // row), bits 1,3,5,7 = north bonds from the previous row into sites 0..3; bit 6 unused (0)
+    uint32_t a[128][4];    // index: bits 0,2,4 = E0,E1,E2 (east bonds site j -> j+1 of this row), bits 1,3,5,6 = north bonds
+                           // from the previous row into sites 0..3 (the bond byte with bit 7 moved to bit 6)
     uint32_t b[128];       // index: bits 0,2,4,6 = E0..E3 (E3 = east bond into the next lane), bit 1 = EL (link from the
                            // previous lane)
 };
@@ -32,9 +32,9 @@ struct ScanLut {
 constexpr ScanLut make_scan_lut()
 {
     ScanLut t{};
-    for (int i = 0; i < 256; ++i) {
+    for (int i = 0; i < 128; ++i) {
         const bool E0 = i & 1, E1 = i & 4, E2 = i & 16;
-        const int np = ((i >> 1) & 1) | (((i >> 3) & 1) << 1) | (((i >> 5) & 1) << 2) | (((i >> 7) & 1) << 3);
+        const int np = ((i >> 1) & 1) | (((i >> 3) & 1) << 1) | (((i >> 5) & 1) << 2) | (((i >> 6) & 1) << 3);
         int s[4] = {0, 0, 0, 0};                         // first site of each site's segment (run inside the lane)
         s[1] = E0 ? 0 : 1;
         s[2] = E1 ? s[1] : 2;
@@ -57,7 +57,7 @@ constexpr ScanLut make_scan_lut()
         const uint32_t m01 = lut_sel((np & 1) ? 0 : 1, (np & 2) ? 0 : 1);
         const uint32_t m23 = lut_sel((np & 4) ? 0 : 1, (np & 8) ? 0 : 1);
         int cnt = 0;                                     // active bonds in the pattern
-        for (int k = 0; k < 8; ++k) cnt += (i >> k) & 1;
+        for (int k = 0; k < 7; ++k) cnt += (i >> k) & 1;
         t.a[i][0] = selX | (selL01 << 16);
         t.a[i][1] = selW | (selL23 << 16);
         t.a[i][2] = m01 | (m23 << 16);
@@ -135,9 +135,9 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
 {
     __shared__ __align__(16) uint16_t s_nm[SCAN_WARPS][TW * TH];
     __shared__ uint32_t s_q[SCAN_WARPS][QCAP];
-    __shared__ __align__(16) uint4 s_la[256];
+    __shared__ __align__(16) uint4 s_la[128];
     __shared__ uint32_t s_lb[128];
-    for (int i = threadIdx.x; i < 256; i += SCAN_THREADS)
+    for (int i = threadIdx.x; i < 128; i += SCAN_THREADS)
         s_la[i] = make_uint4(d_scan_lut.a[i][0], d_scan_lut.a[i][1], d_scan_lut.a[i][2], d_scan_lut.a[i][3]);
     for (int i = threadIdx.x; i < 128; i += SCAN_THREADS) s_lb[i] = d_scan_lut.b[i];
     __syncthreads();                                     // the only block-wide barrier
@@ -181,7 +181,7 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
     }
 
     uint32_t P01 = 0, P23 = 0;                           // names carried by the previous row's sites
-    uint32_t npm = 0;                                    // north bonds from the previous row into this row (bits 1,3,5,7)
+    uint32_t npm = 0;                                    // north bonds from the previous row into this row (bits 1,3,5,6)
     uint32_t NEW01 = (uint32_t)(4 * lane) * 0x00010001u + 0x00010000u;      // own names of sites 0,1 / 2,3 of this row
     uint32_t NEW23 = NEW01 + 0x00020002u;
     uint32_t nact = 0;
@@ -293,7 +293,7 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
         }
 
         P01 = l01; P23 = l23;
-        npm = G & 0xAAu;
+        npm = (G & 0x2Au) | ((G >> 1) & 0x40u);
         NEW01 += (uint32_t)TW * 0x00010001u;
         NEW23 += (uint32_t)TW * 0x00010001u;
         gi += L;
