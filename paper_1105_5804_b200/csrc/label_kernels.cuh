@@ -332,7 +332,8 @@ k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __rest
     // (4) every site
     const int r0 = MODE == MODE_WOLFF ? sm.r0 : -1;
     const int lmask = (1 << p.sbit) - 1;
-    const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(sm.S);
+    uint32_t sbase = (uint32_t)__cvta_generic_to_shared(sm.S);
+    asm volatile("mov.u32 %0, %0;" : "+r"(sbase));       // keep it in a register (ptxas would recompute it at every use)
     const uint32_t sshift = (uint32_t)p.sbit - 24u, smask = 0x01010101u * ((1u << (31 - p.sbit)) - 1u);
     int nflip = 0;
     int* lrow = labels + (size_t)(y0 + ly0) * L + x;
