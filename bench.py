@@ -29,8 +29,12 @@ BYTES_PER_SITE_SWEEP = 14.0      # SURVEY 8(d) model (iii) / DESIGN.md: 1 + 4 + 
 BYTES_PER_SITE = {"k_scan": 5.0, "k_seam": 0.0, "k_final": 9.0}   # DESIGN.md per-kernel table
 PHASES = ["k_scan", "k_seam", "k_final"]
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture
-# (profiles/r01_ncu_full.md), bytes; None until a capture exists for that kernel.
-NCU_TRAFFIC = {"k_scan": None, "k_final": None}
+# (profiles/r01c_README.md), bytes, at L=16384 beta_c; None for other sizes.
+NCU_TRAFFIC = {"k_scan": 0.269366e9 + 1.101867e9, "k_seam": 0.328653e9 + 0.052963e9, "k_final": 1.073979e9 + 1.282681e9}
+# smsp__inst_executed.sum per launch from the same capture: the kernels are instruction-issue bound
+NCU_WARP_INST = {"k_scan": 810.58e6, "k_seam": 38.71e6, "k_final": 451.44e6}
+N_SMSP = 148 * 4
+BYTES_PER_SITE_LABEL = 12.25     # sw_label alone = packed bonds 0.25 + 4 + 4 + 4
 
 
 def beta_c_ising() -> float:
@@ -212,6 +216,57 @@ def run_ours(args):
     per_kernel = {name: phase_ms[i] / max(1, nprof) for i, name in enumerate(PHASES)}
     obs = lat.observables()
 
+    # ---- labelling alone (BASELINE.json configs[3], metric "labelling GB/s"): bond percolation at p = 1/2 --------------
+    labelling = None
+    if rank == 0 and not args.no_labelling:
+        latp = binding.Lattice(L, 2, beta, 1, device=device, with_bonds=True)
+        latp.init_spins(0)                                            # cold spins: every bond is satisfied
+        latp.set_threshold(1 << 31)                                   # floor(0.5 * 2^32): each bond open with p = 1/2
+        latp.activate()
+        for _ in range(3):
+            latp.label()
+        torch.cuda.synchronize()
+        nrep = 20
+        ev0.record(stream)
+        for _ in range(nrep):
+            latp.label()
+        ev1.record(stream)
+        torch.cuda.synchronize()
+        lab_ms = ev0.elapsed_time(ev1) / nrep
+        latp.profile_enable(True)
+        for _ in range(nrep):
+            latp.label()
+        lab_phase, nlab = latp.profile_read()
+        latp.profile_enable(False)
+        cs = latp.cluster_stats()
+        peak_l, _ = measured_peak_gbs()
+        gbs = BYTES_PER_SITE_LABEL * N / (lab_ms * 1e-3) / 1e9
+        labelling = {"workload": "sw_label on i.i.d. bonds, p=0.5, L=%d (packed bonds -> canonical int32 labels)" % L,
+                     "ms": lab_ms, "ns_per_site": lab_ms * 1e6 / N, "algorithmic_bytes_per_site": BYTES_PER_SITE_LABEL,
+                     "GB/s": gbs, "frac_of_measured_peak": gbs / peak_l, "frac_of_8TBps_nominal": gbs / 8000.0,
+                     "kernel_ms": {name: lab_phase[i] / max(1, nlab) for i, name in enumerate(PHASES)},
+                     "clusters_per_site": cs["n_clusters"] / N}
+        latp.close()
+
+    # ---- the other temperatures of BASELINE.json configs[2] (short runs; the headline stays beta_c) -------------------
+    other_betas = None
+    if rank == 0 and args.all_betas:
+        other_betas = {}
+        for b in (0.40, 0.50):
+            lb = binding.Lattice(L, 2, b, 1, device=device)
+            lb.init_spins(1)
+            lb.sweep(60)
+            torch.cuda.synchronize()
+            ev0.record(stream)
+            lb.sweep(40)
+            ev1.record(stream)
+            torch.cuda.synchronize()
+            ms = ev0.elapsed_time(ev1) / 40
+            lb.profile_enable(True); lb.sweep(20); ph, nb = lb.profile_read(); lb.profile_enable(False)
+            other_betas["%.2f" % b] = {"ms_per_step": ms, "ns_per_spin_update": ms * 1e6 / N,
+                                       "kernel_ms": {name: ph[i] / max(1, nb) for i, name in enumerate(PHASES)}}
+            lb.close()
+
     # ---- end to end through the host-buffer entry point ----------------------------------------------------
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
     h_in = torch.empty(N, dtype=torch.int8).pin_memory()
@@ -240,7 +295,7 @@ def run_ours(args):
     dom_bytes = BYTES_PER_SITE[dom] * N
     achieved = dom_bytes / (per_kernel[dom] * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": NCU_TRAFFIC.get(dom), "peak_source": peak_src,
+                "frac": achieved / peak, "traffic": NCU_TRAFFIC.get(dom) if L == 16384 else None, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": dom_bytes, "kernel_ms": per_kernel[dom],
                 "kernel_ms_all": per_kernel,
                 "kernel_share_of_step": per_kernel[dom] / max(1e-12, sum(per_kernel.values())),
@@ -249,6 +304,12 @@ def run_ours(args):
                           "frac_of_measured_peak": BYTES_PER_SITE_SWEEP * N / (ms_per_step * 1e-3) / 1e9 / peak,
                           "frac_of_8TBps_nominal": BYTES_PER_SITE_SWEEP * N / (ms_per_step * 1e-3) / 1e9 / 8000.0,
                           "frac_compulsory_6B_of_measured_peak": 6.0 * N / (ms_per_step * 1e-3) / 1e9 / peak}}
+
+    if L == 16384 and clocks and clocks.get("sm_mhz"):
+        # issue-slot view: warp instructions per launch (ncu) / (SM sub-partitions x clock x kernel time); peak 1 per cycle
+        roofline["alu"] = {name: {"warp_inst": NCU_WARP_INST[name],
+                                  "issue_frac": NCU_WARP_INST[name] / (N_SMSP * clocks["sm_mhz"] * 1e6 * per_kernel[name] * 1e-3)}
+                           for name in PHASES}
 
     # ---- the oracle on this box's host cores, bounded sample ---------------------------------------------------
     cpu = None
@@ -261,7 +322,7 @@ def run_ours(args):
         lat_s.close()
         import oracle
         T = oracle.threshold(2, beta)
-        nsw = 4 if Ls >= 4096 else 8
+        nsw = 12 if Ls >= 4096 else 24
         t0 = time.perf_counter()
         for k in range(nsw):
             oracle.sweep(Ls, 2, T, 1, 60 + k, s)
@@ -289,6 +350,8 @@ def run_ours(args):
         "gpu_launches": launches,
         "roofline": roofline,
         "cpu_baseline": cpu,
+        "labelling": labelling,
+        "other_betas": other_betas,
         "state": {"energy_per_site": obs["energy"] / N, "magnetisation_per_site": obs["magnetisation"] / N,
                   "clusters_per_site": obs["n_clusters"] / N, "largest_cluster_fraction": obs["max_cluster"] / N,
                   "counter": obs["counter"]},
@@ -310,6 +373,8 @@ def main(argv=None):
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-labelling", action="store_true")
+    ap.add_argument("--all-betas", action="store_true")
     args = ap.parse_args(argv)
     if args.warmup < 3:
         args.warmup = 3
