@@ -90,39 +90,54 @@ k_observables(const Params p, const uint32_t* __restrict__ spins_w, Acc* __restr
     }
 }
 
-// S:8a a9: size[r] = number of sites with label r.  Equal labels in consecutive sites are merged in registers, then
-// across the warp with match_any, so that a giant cluster costs one atomic per warp instead of one per site.
+// S:8a a9 (P:142 sizes kept in the roots): size[r] += number of sites labelled r.  One CTA per TW x TH strip: the sites of
+// a strip carry few distinct labels (one per cluster that enters the strip), so they are first counted in a shared-memory
+// hash table (open addressing, as many slots as sites: it cannot overflow) and every distinct label of the strip costs ONE
+// global atomic -- the giant cluster at beta_c gets one atomic per strip instead of one per site.  Equal neighbours inside
+// a thread's 4 sites are merged before the table is touched.
+constexpr int CS_SLOTS = TW * TH;
 __global__ void __launch_bounds__(256)
 k_cluster_sizes(const Params p, const int* __restrict__ labels, int* __restrict__ size)
 {
-    const int nv = p.N >> 2;
-    for (int i4 = blockIdx.x * blockDim.x + threadIdx.x; i4 < ((nv + 31) & ~31); i4 += gridDim.x * blockDim.x) {
-        int lab[4] = {-1, -2, -3, -4};
-        int cnt[4] = {0, 0, 0, 0};
-        if (i4 < nv) {
-            const int4 v = reinterpret_cast<const int4*>(labels)[i4];
-            lab[0] = v.x; lab[1] = v.y; lab[2] = v.z; lab[3] = v.w;
-            cnt[0] = cnt[1] = cnt[2] = cnt[3] = 1;
+    __shared__ int s_key[CS_SLOTS];
+    __shared__ int s_cnt[CS_SLOTS];
+    const int L = p.L;
+    const int x0 = blockIdx.x * TW, y0 = blockIdx.y * TH;
+    for (int i = threadIdx.x; i < CS_SLOTS; i += blockDim.x) { s_key[i] = -1; s_cnt[i] = 0; }
+    __syncthreads();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+    const int x = x0 + 4 * lane;
+    if (x < L) {
+        for (int ly = warp; ly < TH && y0 + ly < L; ly += nwarp) {
+            const int4 v = *reinterpret_cast<const int4*>(labels + (size_t)(y0 + ly) * L + x);
+            int lab[4] = {v.x, v.y, v.z, v.w};
+            int cnt[4] = {1, 1, 1, 1};
 #pragma unroll
             for (int j = 1; j < 4; ++j)
                 if (lab[j] == lab[j - 1]) { cnt[j] += cnt[j - 1]; cnt[j - 1] = 0; }
-        }
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const int key = cnt[j] ? lab[j] : -1 - (int)(threadIdx.x & 31) - 32 * j;   // inactive: unique key
-            const uint32_t peers = __match_any_sync(0xffffffffu, key);
-            int tot = 0;
-            for (uint32_t m = peers; m; m &= m - 1) tot += __shfl_sync(peers, cnt[j], __ffs(m) - 1);
-            if (cnt[j] && (threadIdx.x & 31) == (uint32_t)(__ffs(peers) - 1)) atomicAdd(&size[key], tot);
+            for (int j = 0; j < 4; ++j) {
+                if (cnt[j] == 0) continue;
+                uint32_t slot = ((uint32_t)lab[j] * 0x9E3779B1u) >> (32 - TW_LOG - TH_LOG);
+                while (true) {
+                    const int old = atomicCAS(&s_key[slot], -1, lab[j]);
+                    if (old == -1 || old == lab[j]) break;
+                    slot = (slot + 1) & (CS_SLOTS - 1);
+                }
+                atomicAdd(&s_cnt[slot], cnt[j]);
+            }
         }
     }
+    __syncthreads();
+    for (int i = threadIdx.x; i < CS_SLOTS; i += blockDim.x)
+        if (s_key[i] >= 0) atomicAdd(&size[s_key[i]], s_cnt[i]);
 }
 
 // Statistics over the roots (labels[i] == i): count, maximum, sum of squares, log2-binned histogram.
 __global__ void __launch_bounds__(256)
 k_cluster_stats(const Params p, const int* __restrict__ labels, const int* __restrict__ size, Acc* __restrict__ acc)
 {
-    __shared__ unsigned long long s_hist[32];
+    __shared__ unsigned int s_hist[32];                  // per-CTA counts fit 32 bits (native shared-memory atomics)
     __shared__ unsigned long long s_n, s_max, s_sq;
     if (threadIdx.x < 32) s_hist[threadIdx.x] = 0;
     if (threadIdx.x == 0) { s_n = 0; s_max = 0; s_sq = 0; }
@@ -134,7 +149,7 @@ k_cluster_stats(const Params p, const int* __restrict__ labels, const int* __res
             ++n;
             mx = s > mx ? s : mx;
             sq += s * s;
-            atomicAdd(&s_hist[31 - __clz((unsigned)s)], 1ull);
+            atomicAdd(&s_hist[31 - __clz((unsigned)s)], 1u);
         }
     }
     n = warp_sum_u64(n);
@@ -150,7 +165,7 @@ k_cluster_stats(const Params p, const int* __restrict__ labels, const int* __res
         atomicMax(&s_max, mx);
     }
     __syncthreads();
-    if (threadIdx.x < 32 && s_hist[threadIdx.x]) atomicAdd(&acc->hist[threadIdx.x], s_hist[threadIdx.x]);
+    if (threadIdx.x < 32 && s_hist[threadIdx.x]) atomicAdd(&acc->hist[threadIdx.x], (unsigned long long)s_hist[threadIdx.x]);
     if (threadIdx.x == 0) {
         if (s_n) atomicAdd(&acc->cs_nclusters, s_n);
         if (s_sq) atomicAdd(&acc->cs_sumsq, s_sq);

@@ -8,8 +8,8 @@
 // busy) in the strip's forest.  Names never depend on the forest, so the row loop has no divergent part.
 //
 // Names are strip-local site indices (< TW*TH = 4096) kept as 16-bit halves, two per register: P01/P23 = names carried
-// by the 4 sites of the previous row, l01/l23 = names of this row.  Which name a site takes is a function of 8 bits --
-// the lane's 3 inner east bonds and the 4 north bonds from the row above -- so it comes from a 256-entry table of byte
+// by the 4 sites of the previous row, l01/l23 = names of this row.  Which name a site takes is a function of 7 bits --
+// the lane's 3 inner east bonds and the 4 north bonds from the row above -- so it comes from a 128-entry table of byte
 // permutation selectors (PRMT): 4 permutes name the 4 sites, 2 more (selectors from a second table, indexed by the 4
 // east bonds and the link from the previous lane) substitute the names of runs that cross lane boundaries.
 #pragma once

@@ -332,7 +332,7 @@ static int cluster_stats_device(sw_handle* h, const int32_t* labels, cudaStream_
     const Params p = params_at(h, h->t);
     SW_CUDA(h, cudaMemsetAsync(h->d_size, 0, (size_t)h->N * sizeof(int32_t), s));
     SW_CUDA(h, cudaMemsetAsync(&h->d_acc->cs_nclusters, 0, sizeof(unsigned long long) * (3 + 32), s));
-    k_cluster_sizes<<<grid_capped(h->N / 4, 256, 148 * 16), 256, 0, s>>>(p, labels, h->d_size);
+    k_cluster_sizes<<<dim3(p.ntx, p.nty), 256, 0, s>>>(p, labels, h->d_size);
     SW_LAUNCHED(h, "k_cluster_sizes");
     k_cluster_stats<<<grid_capped(h->N, 256, 148 * 8), 256, 0, s>>>(p, labels, h->d_size, h->d_acc);
     SW_LAUNCHED(h, "k_cluster_stats");
