@@ -229,6 +229,12 @@ def run_ours(args):
         nrep = 20
         ev0.record(stream)
         for _ in range(nrep):
+            latp.activate()                                           # materialised packed bonds (a1 alone)
+        ev1.record(stream)
+        torch.cuda.synchronize()
+        act_ms = ev0.elapsed_time(ev1) / nrep
+        ev0.record(stream)
+        for _ in range(nrep):
             latp.label()
         ev1.record(stream)
         torch.cuda.synchronize()
@@ -245,7 +251,10 @@ def run_ours(args):
                      "ms": lab_ms, "ns_per_site": lab_ms * 1e6 / N, "algorithmic_bytes_per_site": BYTES_PER_SITE_LABEL,
                      "GB/s": gbs, "frac_of_measured_peak": gbs / peak_l, "frac_of_8TBps_nominal": gbs / 8000.0,
                      "kernel_ms": {name: lab_phase[i] / max(1, nlab) for i, name in enumerate(PHASES)},
-                     "clusters_per_site": cs["n_clusters"] / N}
+                     "clusters_per_site": cs["n_clusters"] / N,
+                     "activation_only": {"what": "sw_activate: spins -> packed bonds (1.25 B/site), not on the sweep path "
+                                                 "(a sweep draws its bonds inside k_scan)", "ms": act_ms,
+                                         "ns_per_site": act_ms * 1e6 / N}}
         latp.close()
 
     # ---- the other temperatures of BASELINE.json configs[2] (short runs; the headline stays beta_c) -------------------
