@@ -28,27 +28,26 @@ k_init(const Params p, uint32_t* __restrict__ spins_w, int mode)
     }
 }
 
-// Packed bonds of step t for the current spins (P:70 bond array; S:8c.3-4).  One thread per 4 sites = one byte.
+// Packed bonds of step t for the current spins (P:70 bond array; S:8c.3-4).  One thread per 16 sites = 4 bytes (N/4 is a
+// multiple of 4 because L is), the same draw-to-bit arithmetic as k_scan (scan_kernel.cuh bond_byte).
+template <bool ISING>
 __global__ void __launch_bounds__(256)
 k_activate(const Params p, const uint32_t* __restrict__ spins_w, uint8_t* __restrict__ bonds)
 {
-    const int L = p.L, Lw = L >> 2, nw = p.N >> 2;
-    for (int i4 = blockIdx.x * blockDim.x + threadIdx.x; i4 < nw; i4 += gridDim.x * blockDim.x) {
-        const int yy = i4 / Lw, xw = i4 - yy * Lw;
-        const uint32_t w = spins_w[i4];
-        const uint32_t we = spins_w[yy * Lw + (xw + 1 == Lw ? 0 : xw + 1)];
-        const uint32_t wn = spins_w[(yy + 1 == L ? 0 : yy + 1) * Lw + xw];
-        const uint32_t eqe = eq_bytes4(w, __funnelshift_r(w, we, 8));
-        const uint32_t eqn = eq_bytes4(w, wn);
-        const uint32_t c0 = (uint32_t)i4 * 2u;           // (i>>1) of the first pair of this word
-        uint32_t a0, a1, a2, a3, b0, b1, b2, b3;
-        philox4x32_10(p, c0, p.t_lo, p.t_hi, DOM_BOND, a0, a1, a2, a3);
-        philox4x32_10(p, c0 + 1, p.t_lo, p.t_hi, DOM_BOND, b0, b1, b2, b3);
-        const uint32_t e0 = (eqe & 1u) && a0 < p.T, n0 = (eqn & 1u) && a1 < p.T;
-        const uint32_t e1 = (eqe & 2u) && a2 < p.T, n1 = (eqn & 2u) && a3 < p.T;
-        const uint32_t e2 = (eqe & 4u) && b0 < p.T, n2 = (eqn & 4u) && b1 < p.T;
-        const uint32_t e3 = (eqe & 8u) && b2 < p.T, n3 = (eqn & 8u) && b3 < p.T;
-        bonds[i4] = (uint8_t)(e0 | (n0 << 1) | (e1 << 2) | (n1 << 3) | (e2 << 4) | (n2 << 5) | (e3 << 6) | (n3 << 7));
+    const int L = p.L, Lw = L >> 2, nq = p.N >> 4;
+    for (int i16 = blockIdx.x * blockDim.x + threadIdx.x; i16 < nq; i16 += gridDim.x * blockDim.x) {
+        uint32_t out = 0;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const int i4 = 4 * i16 + k;
+            const int yy = p.logL >= 0 ? (i4 >> (p.logL - 2)) : i4 / Lw, xw = i4 - yy * Lw;
+            const uint32_t w = spins_w[i4];
+            const uint32_t we = spins_w[yy * Lw + (xw + 1 == Lw ? 0 : xw + 1)];
+            const uint32_t wn = spins_w[(yy + 1 == L ? 0 : yy + 1) * Lw + xw];
+            // (i>>1) of the first pair of this word = 2 * i4
+            out |= bond_byte<ISING>(p, (uint32_t)i4 * 2u, w, __funnelshift_r(w, we, 8), wn) << (8 * k);
+        }
+        reinterpret_cast<uint32_t*>(bonds)[i16] = out;
     }
 }
 

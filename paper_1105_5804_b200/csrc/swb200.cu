@@ -300,7 +300,10 @@ int sw_activate(sw_handle* h, void* stream)
     if (!h) return SW_EINVAL;
     if (!h->bound || !h->d_bonds) return SW_ESTATE;
     const Params p = params_at(h, h->t);
-    k_activate<<<grid_capped(h->N / 4, 256, 148 * 16), 256, 0, (cudaStream_t)stream>>>(p, h->d_spins, h->d_bonds);
+    if (h->q == 2)
+        k_activate<true><<<grid_capped(h->N / 16, 256, 148 * 16), 256, 0, (cudaStream_t)stream>>>(p, h->d_spins, h->d_bonds);
+    else
+        k_activate<false><<<grid_capped(h->N / 16, 256, 148 * 16), 256, 0, (cudaStream_t)stream>>>(p, h->d_spins, h->d_bonds);
     SW_LAUNCHED(h, "k_activate");
     return SW_OK;
 }
