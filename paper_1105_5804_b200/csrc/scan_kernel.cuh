@@ -128,7 +128,8 @@ __device__ __forceinline__ uint32_t bond_byte(const Params& p, uint32_t c0, uint
 // ---------------------------------------------------------------------------------------------------- k_scan
 // FROM_BONDS=false: read spins, draw bonds (a1).  FROM_BONDS=true: read packed bonds (sw_label).  Writes the provisional
 // labels (`prov`, see label_kernels.cuh) and the edge arrays, and adds the number of active bonds to acc->n_active.
-template <bool FROM_BONDS, bool ISING>
+// FULLW: L is a multiple of TW, every strip has all 32 lanes (no ragged right edge; the predicates fold away).
+template <bool FROM_BONDS, bool ISING, bool FULLW>
 __global__ void __launch_bounds__(SCAN_THREADS)
 k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __restrict__ bonds_in, int* prov,
        int* __restrict__ edgeA, int* __restrict__ edgeB, Acc* __restrict__ acc)
@@ -150,9 +151,9 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
     volatile uint32_t* q = s_q[warp];
     const int L = p.L, Lw = L >> 2;
     const int x0 = tx * TW, y0 = ty * TH;
-    const int tw_eff = min(TW, L - x0), th_eff = min(TH, L - y0);
+    const int tw_eff = FULLW ? TW : min(TW, L - x0), th_eff = min(TH, L - y0);
     const int x = x0 + 4 * lane;
-    const bool colv = 4 * lane < tw_eff;
+    const bool colv = FULLW || 4 * lane < tw_eff;
     const int last_lane = (tw_eff >> 2) - 1;             // lane that owns the strip's last column
     const bool is_last = lane == last_lane;
     const int base = y0 * L + x0;

@@ -124,10 +124,10 @@ int launch_label_front(sw_handle* h, const Params& p, const uint8_t* bonds, int3
 {
     prof_mark(h, 0, s);
     const dim3 grid((p.ntx + SCAN_WARPS - 1) / SCAN_WARPS, p.nty);
-    if (FROM_BONDS || p.q == 2)
-        k_scan<FROM_BONDS, true><<<grid, SCAN_THREADS, 0, s>>>(p, h->d_spins, bonds, labels, h->d_edgeA, h->d_edgeB, h->d_acc);
-    else
-        k_scan<false, false><<<grid, SCAN_THREADS, 0, s>>>(p, h->d_spins, bonds, labels, h->d_edgeA, h->d_edgeB, h->d_acc);
+    const bool ising = FROM_BONDS || p.q == 2, fullw = (p.L % TW) == 0;
+    auto kern = ising ? (fullw ? k_scan<FROM_BONDS, true, true> : k_scan<FROM_BONDS, true, false>)
+                      : (fullw ? k_scan<false, false, true> : k_scan<false, false, false>);
+    kern<<<grid, SCAN_THREADS, 0, s>>>(p, h->d_spins, bonds, labels, h->d_edgeA, h->d_edgeB, h->d_acc);
     SW_LAUNCHED(h, "k_scan");
     prof_mark(h, 1, s);
     const int nseam = (p.ntx + p.nty) * p.L;
