@@ -151,7 +151,7 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
     volatile uint32_t* q = s_q[warp];
     const int L = p.L, Lw = L >> 2;
     const int x0 = tx * TW, y0 = ty * TH;
-    const int tw_eff = FULLW ? TW : min(TW, L - x0), th_eff = min(TH, L - y0);
+    const int tw_eff = FULLW ? TW : min(TW, L - x0), th_eff = FULLW ? TH : min(TH, L - y0);   // TH divides TW
     const int x = x0 + 4 * lane;
     const bool colv = FULLW || 4 * lane < tw_eff;
     const int last_lane = (tw_eff >> 2) - 1;             // lane that owns the strip's last column
