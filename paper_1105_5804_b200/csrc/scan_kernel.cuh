@@ -186,9 +186,8 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
     uint32_t NEW01 = (uint32_t)(4 * lane) * 0x00010001u + 0x00010000u;      // own names of sites 0,1 / 2,3 of this row
     uint32_t NEW23 = NEW01 + 0x00020002u;
     uint32_t nact = 0;
-    int nlink = 0;                                       // active east bonds between lanes (warp-uniform)
     int qn = 0;                                          // queued pairs (warp-uniform)
-    uint32_t eastm = 0;                                  // last lane: bit (th_eff-1-ly) = the east bond that leaves the strip
+    uint32_t eastm = 0;                                  // bit (th_eff-1-ly) = the east bond of site 3 in row ly (last lane: it leaves the strip)
     uint32_t northm = 0;                                 // bond byte of the last row: its north bonds (bits 1,3,5,7) leave the strip
 
     // running per-row quantities: Philox counter of the lane's first pair, global index of the lane's first site, pointer
@@ -240,7 +239,6 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
         const unsigned FULLB = __ballot_sync(FULLM, (G & 0x15u) == 0x15u);
         const unsigned CS = __ballot_sync(FULLM, (A.w & 1u) != 0u);
         const unsigned CP = __ballot_sync(FULLM, (A.w & 2u) != 0u);
-        nlink += __popc(LINK);
         const unsigned nPTL = ~(FULLB & (LINK << 1));                       // lanes where a run cannot pass to the left
         const unsigned nPTR = ~(FULLB & LINK);                              // ... to the right
         const int a_le = 31 - __clz(nPTL & le);                             // bit 0 of nPTL is always set
@@ -342,10 +340,9 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
 
     if (!FROM_BONDS) {
         nact += __popc(northm);
-        if (is_last) nact += __popc(eastm);
+        if (colv) nact += __popc(eastm);                 // my east bonds into the next lane / out of the strip, all rows
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) nact += __shfl_xor_sync(FULLM, nact, o);
-        nact += (uint32_t)nlink;
         if (lane == 0 && nact) atomicAdd(&acc->n_active, (unsigned long long)nact);
     }
 }
