@@ -30,9 +30,9 @@ BYTES_PER_SITE = {"k_scan": 5.0, "k_seam": 0.0, "k_final": 9.0}   # DESIGN.md pe
 PHASES = ["k_scan", "k_seam", "k_final"]
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture
 # (profiles/r01c_README.md), bytes, at L=16384 beta_c; None for other sizes.
-NCU_TRAFFIC = {"k_scan": 0.269366e9 + 1.101867e9, "k_seam": 0.328653e9 + 0.052963e9, "k_final": 1.073979e9 + 1.282681e9}
+NCU_TRAFFIC = {"k_scan": 0.268577e9 + 1.101891e9, "k_seam": 0.328467e9 + 0.053556e9, "k_final": 1.073818e9 + 1.282418e9}
 # smsp__inst_executed.sum per launch from the same capture: the kernels are instruction-issue bound
-NCU_WARP_INST = {"k_scan": 810.58e6, "k_seam": 38.71e6, "k_final": 451.44e6}
+NCU_WARP_INST = {"k_scan": 784.67e6, "k_seam": 38.71e6, "k_final": 421.62e6}
 N_SMSP = 148 * 4
 BYTES_PER_SITE_LABEL = 12.25     # sw_label alone = packed bonds 0.25 + 4 + 4 + 4
 
