@@ -83,7 +83,9 @@ size_t sw_workspace_bytes(int32_t L, int32_t q);
 
 /* Bind caller-owned device buffers: d_spins N bytes (int8 for q=2, uint8 for q>2), d_labels N int32,
  * d_bonds N/4 bytes of packed bonds or NULL (only sw_activate and sw_label(d_bonds=NULL) need it),
- * d_work >= sw_workspace_bytes(L,q) bytes.  Zeroes the accumulators in d_work on `stream`. */
+ * d_work >= sw_workspace_bytes(L,q) bytes.  Zeroes the accumulators in d_work on `stream`: later calls on this
+ * handle must be ordered after that memset -- use the same stream, or synchronise `stream` before the first call on
+ * another one.  (An argument the proposed signature of S:8b does not have; DESIGN.md section 1 lists the deviations.) */
 int sw_bind(sw_handle* h, void* d_spins, int32_t* d_labels, uint8_t* d_bonds, void* d_work, size_t work_bytes,
             void* stream);
 
@@ -126,9 +128,18 @@ int sw_cluster_stats(sw_handle* h, const int32_t* d_labels_in, sw_cstats* h_out,
  * step -- in that case the call synchronises `stream` before returning. */
 int wolff_step(sw_handle* h, int64_t n, int64_t* h_sizes, void* stream);
 
-/* Energy, magnetisation, state counts of the current spins and cluster statistics of the current labels, all in
- * int64 (S:8a a6).  Synchronises `stream`. */
+/* Energy, magnetisation, state counts of the current spins and cluster statistics of the last labelling, all in
+ * int64 (S:8a a6).  Synchronises `stream`.  Equals sw_observables_ex(.., SW_OBS_SPINS | SW_OBS_CLUSTERS, ..). */
 int sw_observables(sw_handle* h, sw_obs* h_out, void* stream);
+
+/* The same with a choice of what is computed (fields not asked for are 0):
+ *   SW_OBS_SPINS    sat_bonds, energy, magnetisation, state_count: one read of the spins (Eq. 1)
+ *   SW_OBS_CLUSTERS max_cluster, sum_sq_cluster: one pass over the labels buffer the last labelling wrote (for a
+ *                   sw_label into a caller buffer that buffer must still be alive)
+ * n_clusters, n_active_bonds and counter are always reported (the labelling counts them itself).  flags = 0 is
+ * valid: it only reads the counters back.  Synchronises `stream`. */
+enum { SW_OBS_SPINS = 1, SW_OBS_CLUSTERS = 2 };
+int sw_observables_ex(sw_handle* h, sw_obs* h_out, int flags, void* stream);
 
 /* Host-buffer convenience for end-to-end use: copy h_spins_in (N bytes, may be NULL to keep the device state)
  * to the device, run n sweeps, copy spins back to h_spins_out (may be NULL) and labels to h_labels_out (may be

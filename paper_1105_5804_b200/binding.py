@@ -13,13 +13,14 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libswb200.so")
 
 SW_OK, SW_EINVAL, SW_ESTATE, SW_ECUDA, SW_ENOMEM = 0, -1, -2, -3, -4
+OBS_SPINS, OBS_CLUSTERS = 1, 2                            # SW_OBS_* of include/swb200.h
 NPHASE = 3                                                # SW_NPHASE of include/swb200.h
 
 # every symbol include/swb200.h declares (tests check that the library exports all of them)
 SYMBOLS = [
     "sw_create", "sw_destroy", "sw_workspace_bytes", "sw_bind", "sw_set_threshold", "sw_get_threshold",
     "sw_set_counter", "sw_get_counter", "sw_init_spins", "sw_sweep", "sw_activate", "sw_label",
-    "sw_cluster_stats", "wolff_step", "sw_observables", "sw_sweep_host", "sw_launch_count", "sw_strerror",
+    "sw_cluster_stats", "wolff_step", "sw_observables", "sw_observables_ex", "sw_sweep_host", "sw_launch_count", "sw_strerror",
     "sw_last_cuda_error", "sw_profile_enable", "sw_profile_read",
 ]
 
@@ -53,9 +54,9 @@ def lib():
     global _lib
     if _lib is not None:
         return _lib
-    if not os.path.exists(LIB_PATH):
-        from . import build as _build
-        _build.build()                                    # raises if nvcc is missing
+    from . import build as _build
+    if not os.path.exists(LIB_PATH) or (_build.needs_build() and _build.have_nvcc()):
+        _build.build()                                    # raises if nvcc is missing; a no-op when up to date
     L = C.CDLL(LIB_PATH)
     vp, i32, i64, u32, u64 = C.c_void_p, C.c_int32, C.c_int64, C.c_uint32, C.c_uint64
     L.sw_create.argtypes = [C.POINTER(vp), i32, i32, C.c_double, u64]
@@ -74,6 +75,7 @@ def lib():
     L.sw_cluster_stats.argtypes = [vp, vp, C.POINTER(sw_cstats), vp]
     L.wolff_step.argtypes = [vp, i64, C.POINTER(i64), vp]
     L.sw_observables.argtypes = [vp, C.POINTER(sw_obs), vp]
+    L.sw_observables_ex.argtypes = [vp, C.POINTER(sw_obs), C.c_int, vp]
     L.sw_sweep_host.argtypes = [vp, vp, i64, vp, vp, C.POINTER(sw_obs), vp]
     L.sw_launch_count.argtypes = [vp, C.POINTER(u64)]
     L.sw_profile_enable.argtypes = [vp, C.c_int]
@@ -184,9 +186,13 @@ class Lattice:
         self._check(self._lib.wolff_step(self._h, n, None, self._stream()))
         return None
 
-    def observables(self) -> dict:
+    def observables(self, spins: bool = True, clusters: bool = True) -> dict:
         out = sw_obs()
-        self._check(self._lib.sw_observables(self._h, C.byref(out), self._stream()))
+        if spins and clusters:
+            self._check(self._lib.sw_observables(self._h, C.byref(out), self._stream()))
+        else:
+            flags = (OBS_SPINS if spins else 0) | (OBS_CLUSTERS if clusters else 0)
+            self._check(self._lib.sw_observables_ex(self._h, C.byref(out), flags, self._stream()))
         return out.as_dict()
 
     def sweep_host(self, h_spins_in, n: int, h_spins_out=None, h_labels_out=None, want_obs: bool = True):

@@ -27,6 +27,14 @@ def _nvcc() -> str:
     raise RuntimeError("nvcc not found: the CUDA library cannot be built and there is no CPU fallback")
 
 
+def have_nvcc() -> bool:
+    try:
+        _nvcc()
+        return True
+    except RuntimeError:
+        return False
+
+
 def sources():
     return sorted(glob.glob(os.path.join(CSRC, "*.cu")))
 

@@ -33,7 +33,7 @@ struct sw_handle {
     int32_t*  d_edgeB;             // (ntx+nty)*L: strip-local roots of first columns / first rows
     int32_t*  d_size;              // N int32
     bool      bound;
-    bool      have_labels;         // a labelling has happened since bind
+    const int32_t* last_labels;    // labels buffer written by the LAST sweep / step / sw_label (NULL: none since bind)
     uint64_t  launches;
     char      cuda_err[256];
     // optional per-kernel timing (sw_profile_*)
@@ -110,10 +110,17 @@ Params params_at(const sw_handle* h, uint64_t t)
 }
 
 constexpr int PROF_MAX = 512;
-inline void prof_mark(sw_handle* h, int phase, cudaStream_t s)
+inline int prof_mark(sw_handle* h, int phase, cudaStream_t s)
 {
-    if (h->prof_on && h->prof_n < PROF_MAX) cudaEventRecord(h->prof_ev[h->prof_n * (SW_NPHASE + 1) + phase], s);
+    if (h->prof_on && h->prof_n < PROF_MAX)
+        SW_CUDA(h, cudaEventRecord(h->prof_ev[h->prof_n * (SW_NPHASE + 1) + phase], s));
+    return SW_OK;
 }
+#define SW_PROF(h, phase, s)                                                 \
+    do {                                                                     \
+        int rc__ = prof_mark((h), (phase), (s));                             \
+        if (rc__) return rc__;                                               \
+    } while (0)
 
 inline int grid_for(int64_t n, int block) { return (int)((n + block - 1) / block); }
 inline int grid_capped(int64_t n, int block, int cap) { int g = grid_for(n, block); return g < cap ? (g < 1 ? 1 : g) : cap; }
@@ -122,18 +129,18 @@ inline int grid_capped(int64_t n, int block, int cap) { int g = grid_for(n, bloc
 template <bool FROM_BONDS>
 int launch_label_front(sw_handle* h, const Params& p, const uint8_t* bonds, int32_t* labels, cudaStream_t s)
 {
-    prof_mark(h, 0, s);
+    SW_PROF(h, 0, s);
     const dim3 grid((p.ntx + SCAN_WARPS - 1) / SCAN_WARPS, p.nty);
     const bool ising = FROM_BONDS || p.q == 2, fullw = (p.L % TW) == 0;
     auto kern = ising ? (fullw ? k_scan<FROM_BONDS, true, true> : k_scan<FROM_BONDS, true, false>)
                       : (fullw ? k_scan<false, false, true> : k_scan<false, false, false>);
     kern<<<grid, SCAN_THREADS, 0, s>>>(p, h->d_spins, bonds, labels, h->d_edgeA, h->d_edgeB, h->d_acc);
     SW_LAUNCHED(h, "k_scan");
-    prof_mark(h, 1, s);
+    SW_PROF(h, 1, s);
     const int nseam = (p.ntx + p.nty) * p.L;
     k_seam<<<grid_for(seam_part(nseam), 256), 256, 0, s>>>(p, h->d_edgeA, h->d_edgeB, labels);
     SW_LAUNCHED(h, "k_seam");
-    prof_mark(h, 2, s);
+    SW_PROF(h, 2, s);
     return SW_OK;
 }
 
@@ -252,7 +259,7 @@ int sw_bind(sw_handle* h, void* d_spins, int32_t* d_labels, uint8_t* d_bonds, vo
     h->d_edgeB = (int32_t*)(h->d_work + w.edgeB);
     h->d_size = (int32_t*)(h->d_work + w.size);
     h->bound = false;
-    h->have_labels = false;
+    h->last_labels = nullptr;
     SW_CUDA(h, cudaMemsetAsync(h->d_work, 0, w.edgeA, (cudaStream_t)stream));
     h->bound = true;
     return SW_OK;
@@ -287,10 +294,10 @@ int sw_sweep(sw_handle* h, int64_t n, void* stream)
         if (rc) return rc;
         k_final<MODE_SW><<<dim3(p.ntx, p.nty), FIN_THREADS, 0, s>>>(p, h->d_labels, h->d_spins, h->d_acc, nullptr);
         SW_LAUNCHED(h, "k_final<SW>");
-        prof_mark(h, 3, s);
+        SW_PROF(h, 3, s);
         if (h->prof_on && h->prof_n < PROF_MAX) ++h->prof_n;
         ++h->t;
-        h->have_labels = true;
+        h->last_labels = h->d_labels;
     }
     return SW_OK;
 }
@@ -324,9 +331,9 @@ int sw_label(sw_handle* h, const uint8_t* d_bonds_in, int32_t* d_labels_out, voi
     if (rc) return rc;
     k_final<MODE_LABEL><<<dim3(p.ntx, p.nty), FIN_THREADS, 0, s>>>(p, labels, nullptr, h->d_acc, nullptr);
     SW_LAUNCHED(h, "k_final<LABEL>");
-    prof_mark(h, 3, s);
+    SW_PROF(h, 3, s);
     if (h->prof_on && h->prof_n < PROF_MAX) ++h->prof_n;
-    if (labels == h->d_labels) h->have_labels = true;
+    h->last_labels = labels;
     return SW_OK;
 }
 
@@ -380,10 +387,10 @@ int wolff_step(sw_handle* h, int64_t n, int64_t* h_sizes, void* stream)
             k_final<MODE_WOLFF><<<dim3(p.ntx, p.nty), FIN_THREADS, 0, s>>>(p, h->d_labels, h->d_spins, h->d_acc,
                                                                          h->d_wolff + k);
             SW_LAUNCHED(h, "k_final<WOLFF>");
-            prof_mark(h, 3, s);
+            SW_PROF(h, 3, s);
             if (h->prof_on && h->prof_n < PROF_MAX) ++h->prof_n;
             ++h->t;
-            h->have_labels = true;
+            h->last_labels = h->d_labels;
         }
         if (h_sizes) {
             SW_CUDA(h, cudaMemcpyAsync(h_sizes + done, h->d_wolff, sizeof(int64_t) * (size_t)batch,
@@ -395,17 +402,20 @@ int wolff_step(sw_handle* h, int64_t n, int64_t* h_sizes, void* stream)
     return SW_OK;
 }
 
-int sw_observables(sw_handle* h, sw_obs* h_out, void* stream)
+int sw_observables_ex(sw_handle* h, sw_obs* h_out, int flags, void* stream)
 {
-    if (!h || !h_out) return SW_EINVAL;
+    if (!h || !h_out || (flags & ~(SW_OBS_SPINS | SW_OBS_CLUSTERS))) return SW_EINVAL;
     if (!h->bound) return SW_ESTATE;
     cudaStream_t s = (cudaStream_t)stream;
     const Params p = params_at(h, h->t);
-    SW_CUDA(h, cudaMemsetAsync(&h->d_acc->sat, 0, sizeof(unsigned long long) * 9, s));
-    k_observables<<<grid_capped(h->N / 4, 256, 148 * 8), 256, 0, s>>>(p, h->d_spins, h->d_acc);
-    SW_LAUNCHED(h, "k_observables");
-    if (h->have_labels) {
-        int rc = cluster_stats_device(h, h->d_labels, s);
+    if (flags & SW_OBS_SPINS) {
+        SW_CUDA(h, cudaMemsetAsync(&h->d_acc->sat, 0, sizeof(unsigned long long) * 9, s));
+        k_observables<<<grid_capped(h->N / 4, 256, 148 * 8), 256, 0, s>>>(p, h->d_spins, h->d_acc);
+        SW_LAUNCHED(h, "k_observables");
+    }
+    const bool clusters = (flags & SW_OBS_CLUSTERS) && h->last_labels;
+    if (clusters) {
+        int rc = cluster_stats_device(h, h->last_labels, s);
         if (rc) return rc;
     }
     Acc a;
@@ -413,27 +423,36 @@ int sw_observables(sw_handle* h, sw_obs* h_out, void* stream)
     SW_CUDA(h, cudaStreamSynchronize(s));
     memset(h_out, 0, sizeof(*h_out));
     const int64_t N = h->N;
-    h_out->sat_bonds = (int64_t)a.sat;
-    int64_t rest = 0;
-    for (int k = 1; k < h->q; ++k) { h_out->state_count[k] = (int64_t)a.cnt[k]; rest += (int64_t)a.cnt[k]; }
-    h_out->state_count[0] = N - rest;
-    if (h->q == 2) {
-        h_out->energy = -(2 * h_out->sat_bonds - 2 * N);
-        h_out->magnetisation = h_out->state_count[0] - h_out->state_count[1];
-    } else {
-        int64_t mx = 0;
-        for (int k = 0; k < h->q; ++k) if (h_out->state_count[k] > mx) mx = h_out->state_count[k];
-        h_out->energy = -h_out->sat_bonds;
-        h_out->magnetisation = (int64_t)h->q * mx - N;
+    if (flags & SW_OBS_SPINS) {
+        h_out->sat_bonds = (int64_t)a.sat;
+        int64_t rest = 0;
+        for (int k = 1; k < h->q; ++k) { h_out->state_count[k] = (int64_t)a.cnt[k]; rest += (int64_t)a.cnt[k]; }
+        h_out->state_count[0] = N - rest;
+        if (h->q == 2) {
+            h_out->energy = -(2 * h_out->sat_bonds - 2 * N);
+            h_out->magnetisation = h_out->state_count[0] - h_out->state_count[1];
+        } else {
+            int64_t mx = 0;
+            for (int k = 0; k < h->q; ++k) if (h_out->state_count[k] > mx) mx = h_out->state_count[k];
+            h_out->energy = -h_out->sat_bonds;
+            h_out->magnetisation = (int64_t)h->q * mx - N;
+        }
     }
-    if (h->have_labels) {
+    if (h->last_labels) {                                // counted by the labelling itself: free
         h_out->n_clusters = (int64_t)a.n_clusters;
         h_out->n_active_bonds = (int64_t)a.n_active;
+    }
+    if (clusters) {
         h_out->max_cluster = (int64_t)a.cs_max;
         h_out->sum_sq_cluster = a.cs_sumsq;
     }
     h_out->counter = h->t;
     return SW_OK;
+}
+
+int sw_observables(sw_handle* h, sw_obs* h_out, void* stream)
+{
+    return sw_observables_ex(h, h_out, SW_OBS_SPINS | SW_OBS_CLUSTERS, stream);
 }
 
 int sw_sweep_host(sw_handle* h, const void* h_spins_in, int64_t n, void* h_spins_out, int32_t* h_labels_out,

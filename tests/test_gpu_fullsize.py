@@ -66,32 +66,138 @@ def one_oracle_sweep_from_gpu_state(lat, L, q, seed, t):
     return o
 
 
-def test_config3_L16384_beta_c_one_sweep_from_gpu_state():
-    """BASELINE.json configs[2] at beta_c, the workload bench.py times: sweeps 0 and 3 against the oracle."""
+def sweep_with_bond_end_check(lat, L):
+    """One GPU sweep whose labels are checked against the bonds of that very step: sw_activate materialises the bond
+    set of step t (same draws as the sweep's own, reading 16), the sweep labels it, and both ends of every
+    active bond must carry one label -- a union lost to a race cannot pass this (the invariants alone could)."""
+    lat.activate()
+    lat.sweep(1)
+    o = lat.observables()
+    assert check_label_properties(L, lat.labels, lat.bonds) == o["n_clusters"]
+    assert int(popcount_bytes(lat.bonds)) == o["n_active_bonds"]
+    return o
+
+
+def popcount_bytes(t):
+    x = t.to(torch.int32)
+    x = (x & 0x55) + ((x >> 1) & 0x55)
+    x = (x & 0x33) + ((x >> 2) & 0x33)
+    x = (x & 0x0F) + (x >> 4)
+    return x.sum(dtype=torch.int64)
+
+
+def test_config3_L16384_beta_c_sampled_sweeps_vs_oracle():
+    """BASELINE.json configs[2] at beta_c, the workload bench.py times: the sampled sweeps {0, 1, 2, 50, 199} of
+    SURVEY.md 8(d) "parity at L=16384", each one oracle sweep from the GPU state.  By sweep 199 the largest cluster holds
+    a quarter of the lattice and spans thousands of strips: the contention of the timed state."""
     L, seed = 16384, 1
-    lat = binding.Lattice(L, 2, BETA_C, seed)
+    lat = binding.Lattice(L, 2, BETA_C, seed, with_bonds=True)
     assert lat.get_threshold() == oracle.threshold(2, BETA_C) == 2515933592
     lat.init_spins(1)
     assert oracle.fnv1a64(lat.spins_host()) == oracle.fnv1a64(oracle.init_spins(L, 2, seed, 1))
-    one_oracle_sweep_from_gpu_state(lat, L, 2, seed, 0)               # from the random start
-    lat.sweep(2)
-    o = one_oracle_sweep_from_gpu_state(lat, L, 2, seed, 3)
+    for t in (0, 1, 2):
+        one_oracle_sweep_from_gpu_state(lat, L, 2, seed, t)
+    lat.sweep(47)
+    o = one_oracle_sweep_from_gpu_state(lat, L, 2, seed, 50)
     assert check_label_properties(L, lat.labels) == o["n_clusters"]
+    lat.sweep(147)
+    sweep_with_bond_end_check(lat, L)                                  # sweep 198, on the device
+    o = one_oracle_sweep_from_gpu_state(lat, L, 2, seed, 199)
+    st = lat.cluster_stats()
+    assert st["max_cluster"] == o["max_cluster"] > 0.1 * L * L         # the giant critical cluster is there
+    lat.close()
+
+
+def test_config3_L16384_beta_c_cold_start_giant_cluster():
+    """Cold start at beta_c: p = 0.586 is above the bond-percolation threshold, so sweep 0 builds one cluster through
+    ~90 % of the lattice and every wrap -- the heaviest root contention the seam pass can see."""
+    L, seed = 16384, 5
+    lat = binding.Lattice(L, 2, BETA_C, seed, with_bonds=True)
+    lat.init_spins(0)
+    o = one_oracle_sweep_from_gpu_state(lat, L, 2, seed, 0)
+    assert o["max_cluster"] > 0.8 * L * L
+    sweep_with_bond_end_check(lat, L)
     lat.close()
 
 
 @pytest.mark.parametrize("beta", [0.40, 0.50])
-def test_config3_L16384_off_critical_properties(beta):
-    """The other temperatures of configs[2]: properties at full size + energy against the exact infinite-lattice value
-    after equilibration is NOT asserted here (40 sweeps are not enough at L=16384); labels and counts are."""
-    L = 16384
-    lat = binding.Lattice(L, 2, beta, 1)
+def test_config3_L16384_off_critical_vs_oracle(beta):
+    """The other temperatures of configs[2]: sweep 50 from the GPU state against the oracle bit for bit, and the
+    bond-end check on the device for the sweep before it."""
+    L, seed = 16384, 1
+    lat = binding.Lattice(L, 2, beta, seed, with_bonds=True)
+    assert lat.get_threshold() == oracle.threshold(2, beta)
     lat.init_spins(1)
-    lat.sweep(4)
-    o = lat.observables()
+    lat.sweep(49)
+    sweep_with_bond_end_check(lat, L)
+    o = one_oracle_sweep_from_gpu_state(lat, L, 2, seed, 50)
     assert check_label_properties(L, lat.labels) == o["n_clusters"]
     st = lat.cluster_stats()
     assert st["n_clusters"] == o["n_clusters"] and sum(st["hist32"]) == o["n_clusters"]
+    if beta == 0.50:
+        assert o["max_cluster"] > 0.5 * L * L                          # ordered phase: one spanning cluster
+    lat.close()
+
+
+@pytest.mark.parametrize("what", ["p=0.5", "p=0.7", "sw beta=0.5"])
+def test_L16384_labelling_repeats_bit_for_bit(what):
+    """compute-sanitizer is closed on this GPU pool, so races are hunted by repetition at the size and contention of
+    the bench: the same packed bonds are labelled 30 times; every result must equal the first (the canonical labelling
+    is unique, reading 7) and the first must satisfy the bond-end check."""
+    L = 16384
+    lat = binding.Lattice(L, 2, 0.5, 3, with_bonds=True)
+    if what.startswith("p="):
+        lat.init_spins(0)
+        lat.set_threshold(oracle.threshold_from_p(float(what[2:])))
+    else:
+        lat.init_spins(1)
+        lat.sweep(30)                                                  # ordered phase: a spanning cluster
+    lat.activate()
+    first = torch.empty(L * L, dtype=torch.int32, device="cuda")
+    lat.label(lat.bonds, first)
+    check_label_properties(L, first, lat.bonds)
+    out = torch.empty_like(first)
+    for rep in range(30):
+        out.fill_(-7)
+        lat.label(lat.bonds, out)
+        assert torch.equal(out, first), "labelling %d of %s differs from the first" % (rep, what)
+    lat.close()
+
+
+def test_L16388_ragged_above_2_28_sites_vs_oracle():
+    """The smallest lattice with N > 2^28: k_final keeps the new state in ONE bit above the label (Params::sbit = 30)
+    and every strip row / column has a ragged last strip.  A few sweeps, then one oracle sweep from the GPU state."""
+    L, seed = 16388, 2
+    lat = binding.Lattice(L, 2, BETA_C, seed, with_bonds=True)
+    lat.init_spins(1)
+    one_oracle_sweep_from_gpu_state(lat, L, 2, seed, 0)
+    lat.sweep(5)
+    sweep_with_bond_end_check(lat, L)
+    o = one_oracle_sweep_from_gpu_state(lat, L, 2, seed, 7)
+    assert check_label_properties(L, lat.labels) == o["n_clusters"]
+    lat.close()
+
+
+def test_L32768_largest_lattice_properties():
+    """The largest lattice the library accepts (N = 2^30, q = 2): init, a few sweeps, canonical-label invariants and the
+    bond-end check on the device, energy moving towards the critical value, cluster statistics consistent."""
+    L = 32768
+    N = L * L
+    lat = binding.Lattice(L, 2, BETA_C, 4, with_bonds=True)
+    lat.init_spins(1)
+    o0 = lat.observables()
+    assert abs(o0["energy"]) < 20 * math.sqrt(2 * N) and abs(o0["magnetisation"]) < 20 * math.sqrt(N)
+    lat.sweep(3)
+    o = sweep_with_bond_end_check(lat, L)
+    assert o["counter"] == 4 and -1.3 * N < o["energy"] < -0.9 * N
+    st = lat.cluster_stats()
+    assert st["n_clusters"] == o["n_clusters"] and sum(st["hist32"]) == o["n_clusters"]
+    assert sum(o["state_count"]) == N
+    # cold start: one cluster through most of the lattice (indices up to 2^30 - 1 on the seam pass)
+    lat.init_spins(0)
+    lat.set_counter(0)
+    o = sweep_with_bond_end_check(lat, L)
+    assert o["max_cluster"] > 0.8 * N
     lat.close()
 
 
