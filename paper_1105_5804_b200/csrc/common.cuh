@@ -22,6 +22,18 @@ constexpr int SCAN_WARPS = SWB_SCAN_WARPS;               // strips per k_scan CT
 constexpr int SCAN_THREADS = 32 * SCAN_WARPS;
 constexpr int FIN_THREADS = SWB_FIN_THREADS;
 constexpr int FIN_WARPS = FIN_THREADS / 32;
+#ifndef SWB_FIN_MIN_CTAS
+#define SWB_FIN_MIN_CTAS (2048 / SWB_FIN_THREADS)
+#endif
+constexpr int FIN_MIN_CTAS = SWB_FIN_MIN_CTAS;
+#ifndef SWB_FIN_MLP
+#define SWB_FIN_MLP 2
+#endif
+constexpr int FIN_MLP = SWB_FIN_MLP;                     // strip-local roots a k_final lane resolves at a time
+#ifndef SWB_GEN_ROWS
+#define SWB_GEN_ROWS 0
+#endif
+constexpr int GEN_ROWS = SWB_GEN_ROWS;                   // rows of every 4 whose bond draws k_final computes one sweep ahead           // resident k_final CTAs per SM the register budget is set for
 static_assert(TW == 128, "lane -> 4 columns, 32 lanes");
 static_assert(TW * TH <= 65536, "strip-local indices are kept in uint16");
 static_assert(TH % FIN_WARPS == 0 && 4 * (TH / FIN_WARPS) <= 32, "k_final keeps one bit per site of a thread in a 32-bit mask");
@@ -38,6 +50,7 @@ struct Params {
     int32_t  ntx, nty;   // number of tile columns / rows
     uint32_t T;          // bond threshold floor(p 2^32)
     uint32_t t_lo, t_hi; // step counter
+    uint32_t u_lo, u_hi; // step counter + 1 (k_final computes the bond draws of the next sweep)
     uint32_t k0[10];     // Philox round keys: k0[r] = seed_lo + r * 0x9E3779B9
     uint32_t k1[10];     //                    k1[r] = seed_hi + r * 0xBB67AE85
     uint32_t negT;       // 2^32 - T (mod 2^32): u + negT carries iff u >= T, for T != 0 (scan_kernel.cuh shift_in_ge)
@@ -85,9 +98,14 @@ __device__ __forceinline__ uint32_t lanemask_lt()
 }
 
 // Device-side accumulators at the start of the workspace (zeroed by sw_bind; parts re-zeroed per call).
-struct Acc {
+constexpr int ACC_PARTS = 32;
+struct AccPart {                       // one 128-byte line per part: same-address atomics serialise in one L2 slice
     unsigned long long n_active;       // bonds activated by the last sweep / step
     unsigned long long n_clusters;     // roots counted by the last flatten pass
+    unsigned long long pad[14];
+};
+struct Acc {
+    AccPart part[ACC_PARTS];           // per-sweep counters: the sum over the parts is the value
     unsigned long long sat;            // observables
     unsigned long long cnt[8];
     unsigned long long cs_nclusters;   // cluster statistics

@@ -121,6 +121,17 @@ __device__ __forceinline__ int gfind(const int* prov, int x)
     return x;
 }
 
+// The same chase in k_final, through the L1 cache: no entry is hooked any more (k_seam has finished; L1 is invalidated at
+// the kernel boundary), the only concurrent writes are final labels -- roots of the same tree -- so a stale line is still
+// an ancestor.  The root entries of the large clusters are read by every strip they pass through: cached per SM they stop
+// being a hot spot in one L2 slice.
+__device__ __forceinline__ int gfind_cached(const int* prov, int x)
+{
+    int pp = __ldca(prov + x);
+    while (pp != x) { x = pp; pp = __ldca(prov + x); }
+    return x;
+}
+
 // Unite the trees of a and b; pa, pb = entries of a and b, loaded by the caller.  Both finds advance in lockstep (two
 // independent loads per round trip), with path halving: nothing more to load when both are roots already, one round
 // trip when each is one hop from its root.
@@ -226,6 +237,8 @@ struct FinalSmem {
     int      S[TW * TH];
     uint16_t list[TW * TH];
     int      r0;
+    int      ncl;                                        // global roots counted by this CTA
+    int      nflip;                                      // sites flipped by this CTA (MODE_WOLFF)
 };
 
 __device__ __forceinline__ int lds_s32(uint32_t saddr)
@@ -246,53 +259,89 @@ __device__ __forceinline__ int lds_s32(uint32_t saddr)
 // only: no block barrier.  (3) every hooked node (each thread looks after its own sites) follows its references to the
 // first entry >= 0 -- the strip-local root or a hooked node that is final already, both carry the final value of the
 // cluster -- and takes that value.  (4) every other site is one hop from a node.
-template <int MODE>
-__global__ void __launch_bounds__(FIN_THREADS, 2048 / FIN_THREADS)
+// GENR > 0: also fill the draw cache (scan_kernel.cuh) with the bond draws of step t+1 for the first GENR rows of every
+// group of 4 rows of this strip: pure integer work that needs no memory, issued while the strip's entries are on their way
+// from HBM.  FULL: no ragged strips (L is a multiple of TW and TH).  Q2: Ising storage (+1 / -1) of the new spins.
+//
+// Flags of a thread's 16 sites (4 rows x 4 columns), one bit per site in a 32-bit word: the site of row r, column j sits
+// at bit 8 j + 7 - 2 r (the top bytes of a row's 4 entries, masked and shifted right by 2 r).
+__device__ __forceinline__ int fin_flag_site(int b)      // bit index -> r * TW + j
+{
+    return (((7 - (b & 7)) >> 1) << TW_LOG) + (b >> 3);
+}
+
+#ifndef SWB_FIN_LDMODE
+#define SWB_FIN_LDMODE 0
+#endif
+#if SWB_FIN_LDMODE == 0
+#define FIN_LD(p) (*(p))
+#elif SWB_FIN_LDMODE == 1
+#define FIN_LD(p) __ldcg(p)
+#else
+#define FIN_LD(p) __ldcs(p)
+#endif
+template <int MODE, int GENR, bool FULL, bool Q2>
+__global__ void __launch_bounds__(FIN_THREADS, FIN_MIN_CTAS)
 k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __restrict__ acc,
-        unsigned long long* __restrict__ wolff_size)
+        unsigned long long* __restrict__ wolff_size, uint32_t* __restrict__ draws)
 {
     __shared__ __align__(16) FinalSmem sm;
     constexpr int R = TH / FIN_WARPS;
+    static_assert(R == 4, "flag words and draw words hold the 4 rows of a warp");
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int L = p.L;
     const int x0 = blockIdx.x * TW, y0 = blockIdx.y * TH;
-    const int tw_eff = min(TW, L - x0);
     const int x = x0 + 4 * lane;
-    const bool colv = 4 * lane < tw_eff;
     const int ly0 = warp * R;
     const int base = y0 * L + x0;
+    const bool colv = FULL || 4 * lane < min(TW, L - x0);
+    const int nrow = FULL ? R : (colv ? max(0, min(R, L - (y0 + ly0))) : 0);   // my valid rows
     volatile int* S = sm.S;
+    int* const lrow0 = labels + (size_t)(y0 + ly0) * L + x;
+    const int l00 = ly0 * TW + 4 * lane;                 // strip-local index of my first site
 
+    if (threadIdx.x == 0) { sm.ncl = 0; sm.nflip = 0; }
     if (MODE == MODE_WOLFF) {
         if (threadIdx.x == 0) {
             uint32_t w0, w1, w2, w3;
             philox4x32_10(p, 0u, p.t_lo, p.t_hi, DOM_WSEED, w0, w1, w2, w3);
             const int i0 = (int)__umulhi(w0, (uint32_t)p.N);
             const int iy = i0 / L, ix = i0 - iy * L;
-            const int b0 = ((iy >> TH_LOG) << TH_LOG) * L + ((ix >> TW_LOG) << TW_LOG);
+            const int b0 = (iy / TH * TH) * L + (ix / TW * TW);
             sm.r0 = gfind(labels, strip_root(labels, L, i0, b0));
         }
     }
 
     // (1) my warp's rows -> shared memory; its roots -> its part of sm.list
-    uint32_t hookm = 0;                                  // bit 4r+j: my site (row r, column j) is a hooked node
+    uint32_t hookw;                                      // flags of my hooked nodes
     uint16_t* const mylist = sm.list + warp * (R * TW);
     int nmine;                                           // roots in my warp's rows
     {
-        uint32_t rootm = 0;                              // ... is a strip-local root
+        int4 vv[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            const int ly = ly0 + r, y = y0 + ly;
-            if (y < L && colv) {
-                const int4 v = *reinterpret_cast<const int4*>(labels + (size_t)y * L + x);
-                *reinterpret_cast<int4*>(&sm.S[ly * TW + 4 * lane]) = v;
-                // top bytes of the 4 entries; bit 7 clear: root, bits 7 and 6 set: hooked node; 4 spread bits -> 4 adjacent
-                const uint32_t t = __byte_perm(__byte_perm(v.x, v.y, 0x0073), __byte_perm(v.z, v.w, 0x0073), 0x5410);
-                rootm |= (((~t & 0x80808080u) * 0x00204081u) >> 28) << (4 * r);
-                hookm |= (((t & (t << 1) & 0x80808080u) * 0x00204081u) >> 28) << (4 * r);
-            }
+            vv[r] = make_int4(REF, REF, REF, REF);       // a site beyond a ragged edge: neither root nor hooked node
+            if (FULL || r < nrow) vv[r] = FIN_LD(reinterpret_cast<const int4*>(lrow0 + (size_t)r * L));
         }
-        const int cnt = __popc(rootm);
+        if (GENR > 0) {
+            uint32_t word = 0;
+            const uint32_t c0 = (uint32_t)((y0 + ly0) * L + x) >> 1;
+#pragma unroll
+            for (int r = 0; r < GENR; ++r)
+                if (FULL || r < nrow) word |= draw_byte(p, c0 + (uint32_t)r * ((uint32_t)L >> 1), p.u_lo, p.u_hi) << (8 * r);
+            draws[draw_word_index(p, blockIdx.x, blockIdx.y, warp, lane)] = word;
+        }
+        uint32_t fl = 0;                                 // REF and HOOK bits of the 16 entries
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int4 v = vv[r];
+            *reinterpret_cast<int4*>(&sm.S[l00 + r * TW]) = v;
+            const uint32_t t = __byte_perm(__byte_perm(v.x, v.y, 0x0073), __byte_perm(v.z, v.w, 0x0073), 0x5410);
+            fl |= (t & 0xC0C0C0C0u) >> (2 * r);
+        }
+        uint32_t rootw = ~fl & 0xAAAAAAAAu;              // REF clear
+        hookw = fl & (fl << 1) & 0xAAAAAAAAu;            // REF and HOOK set
+        const int cnt = __popc(rootw);
         int incl = cnt;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
@@ -300,29 +349,38 @@ k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __rest
             if (lane >= o) incl += t;
         }
         nmine = __shfl_sync(FULLM, incl, 31);
-        int pos = incl - cnt;
-        for (uint32_t m = rootm; m; m &= m - 1) {
-            const int b = __ffs(m) - 1;
-            mylist[pos++] = (uint16_t)((ly0 + (b >> 2)) * TW + 4 * lane + (b & 3));
+        uint16_t* out = mylist + (incl - cnt);
+        const uint32_t tag = (uint32_t)lane << 5;
+        while (rootw) {                                  // entry: flag bit index | lane << 5
+            const int b = 31 - __clz(rootw);
+            rootw ^= 1u << b;
+            *out++ = (uint16_t)(tag | (uint32_t)b);
         }
     }
     __syncwarp();
-    // (2) one global resolve + one Philox draw per strip-local root, balanced over the warp
+    // (2) one global resolve + one Philox draw per strip-local root, balanced over the warp.  The chase over seam-hooked
+    // entries diverges (its length differs from lane to lane); the warp reconverges BEFORE the Philox draw, which would
+    // otherwise be replayed once per chain length.
     int nroots = 0;
     for (int k = lane; k < nmine; k += 32) {
-        const int l = mylist[k];
+        const int code = mylist[k];
+        const int l = ly0 * TW + fin_flag_site(code & 31) + 4 * (code >> 5);
         int v = sm.S[l];
-        const int g = strip_gidx(base, L, l);
-        if (v != g) v = gfind(labels, v);                // hooked by k_seam: find the root of the global tree
+        const int g = base + (l >> TW_LOG) * L + (l & (TW - 1));
+        if (v != g) v = gfind_cached(labels, v);         // hooked by k_seam: find the root of the global tree
+        __syncwarp(__activemask());
         nroots += (v == g);
         // final label and, above bit p.sbit, the new state of the cluster (labels are < 2^sbit)
         sm.S[l] = MODE == MODE_SW ? (int)((uint32_t)v | (flip_state(p, v) << p.sbit)) : v;
     }
+    nroots = __reduce_add_sync(FULLM, nroots);
     __syncthreads();
+    if (lane == 0 && nroots) atomicAdd(&sm.ncl, nroots);
     // (3) my hooked nodes
-    for (uint32_t m = hookm; m; m &= m - 1) {
-        const int b = __ffs(m) - 1;
-        const int l = (ly0 + (b >> 2)) * TW + 4 * lane + (b & 3);
+    while (hookw) {
+        const int b = 31 - __clz(hookw);
+        hookw ^= 1u << b;
+        const int l = l00 + fin_flag_site(b);
         int e = S[l];
         do { e = S[e & LMASK]; } while (e < 0);
         S[l] = e;
@@ -336,22 +394,23 @@ k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __rest
     asm volatile("mov.u32 %0, %0;" : "+r"(sbase));       // keep it in a register (ptxas would recompute it at every use)
     const uint32_t sshift = (uint32_t)p.sbit - 24u, smask = 0x01010101u * ((1u << (31 - p.sbit)) - 1u);
     int nflip = 0;
-    int* lrow = labels + (size_t)(y0 + ly0) * L + x;
+    uint32_t* const srow0 = spins_w + (((size_t)(y0 + ly0) * L + x) >> 2);
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-        const int ly = ly0 + r, y = y0 + ly;
-        if (y < L && colv) {
-            const int4 v = *reinterpret_cast<const int4*>(&sm.S[ly * TW + 4 * lane]);
+        if (FULL || r < nrow) {
+            const int4 v = *reinterpret_cast<const int4*>(&sm.S[l00 + r * TW]);
             int ww[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
             for (int j = 0; j < 4; ++j)                  // not a node: one hop to its node, which is final
                 if (ww[j] < 0) ww[j] = lds_s32(sbase + (((uint32_t)ww[j] << 2) & (uint32_t)(LMASK << 2)));
+            int* const lrow = lrow0 + (size_t)r * L;
+            uint32_t* const srow = srow0 + (size_t)r * (L >> 2);
             if (MODE == MODE_SW) {
                 // the 4 top bytes hold the states above bit sbit - 24
                 const uint32_t t = __byte_perm(__byte_perm(ww[0], ww[1], 0x0073), __byte_perm(ww[2], ww[3], 0x0073), 0x5410);
                 uint32_t word = (t >> sshift) & smask;
-                if (p.q == 2) word = 0x01010101u | (word * 0xFEu);   // k=0 -> +1 (0x01), k=1 -> -1 (0xFF)
-                spins_w[((size_t)y * L + x) >> 2] = word;
+                if (Q2) word = 0x01010101u | (word * 0xFEu);   // k=0 -> +1 (0x01), k=1 -> -1 (0xFF)
+                *srow = word;
                 *reinterpret_cast<int4*>(lrow) = make_int4(ww[0] & lmask, ww[1] & lmask, ww[2] & lmask, ww[3] & lmask);
             } else {
                 *reinterpret_cast<int4*>(lrow) = make_int4(ww[0], ww[1], ww[2], ww[3]);
@@ -360,22 +419,22 @@ k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __rest
                 const uint32_t m = (ww[0] == r0 ? 0xFFu : 0u) | (ww[1] == r0 ? 0xFF00u : 0u) |
                                    (ww[2] == r0 ? 0xFF0000u : 0u) | (ww[3] == r0 ? 0xFF000000u : 0u);   // bytes to negate
                 if (m) {
-                    const uint32_t old = spins_w[((size_t)y * L + x) >> 2];
-                    spins_w[((size_t)y * L + x) >> 2] = __vneg4(old & m) | (old & ~m);
+                    const uint32_t old = *srow;
+                    *srow = __vneg4(old & m) | (old & ~m);
                     nflip += __popc(m) >> 3;
                 }
             }
         }
-        lrow += L;
     }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        nroots += __shfl_xor_sync(FULLM, nroots, o);
-        if (MODE == MODE_WOLFF) nflip += __shfl_xor_sync(FULLM, nflip, o);
-    }
-    if (lane == 0) {
-        if (nroots) atomicAdd(&acc->n_clusters, (unsigned long long)nroots);
-        if (MODE == MODE_WOLFF && nflip) atomicAdd(wolff_size, (unsigned long long)nflip);
+    // one 64-bit atomic per CTA, spread over ACC_PARTS addresses in different 128-byte lines: tens of thousands of atomics
+    // on ONE address serialise in a single L2 slice and stall the whole kernel (measured: 0.71 -> 0.50 ms at beta = 0.5)
+    if (threadIdx.x == 0 && sm.ncl)
+        atomicAdd(&acc->part[(blockIdx.x + 5 * blockIdx.y) & (ACC_PARTS - 1)].n_clusters, (unsigned long long)sm.ncl);
+    if (MODE == MODE_WOLFF) {
+        nflip = __reduce_add_sync(FULLM, nflip);
+        if (lane == 0 && nflip) atomicAdd(&sm.nflip, nflip);
+        __syncthreads();
+        if (threadIdx.x == 0 && sm.nflip) atomicAdd(wolff_size, (unsigned long long)sm.nflip);
     }
 }
 

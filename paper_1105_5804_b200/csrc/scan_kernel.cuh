@@ -101,18 +101,26 @@ __device__ __forceinline__ void shift_in_ge(uint32_t& d, uint32_t u, uint32_t ne
     asm("{\n\t.reg .u32 t;\n\tadd.cc.u32 t, %1, %2;\n\taddc.u32 %0, %0, %0;\n\t}" : "+r"(d) : "r"(u), "r"(negT));
 }
 
-// The lane's bond byte for row y: bit 2j = east bond of site j, bit 2j+1 = north bond of site j (the packed-bond
-// format of include/swb200.h), for the 4 sites whose spins are w; e = spins of the east neighbours, n = of the north.
-template <bool ISING>
-__device__ __forceinline__ uint32_t bond_byte(const Params& p, uint32_t c0, uint32_t w, uint32_t e, uint32_t n)
+// Draw byte of the 4 sites whose first pair has Philox counter c0, at step (t_lo, t_hi): bit 2j = [east draw of site j
+// >= T], bit 2j+1 = [north draw >= T] (S:8c.3: u(i,d,t) = PHILOX(seed; i>>1, t, BOND)[2(i&1)+d]).  A pure function of
+// (seed, t, site, T): k_final computes it one sweep ahead (draw cache, see k_final) and k_scan<SRC_DRAWS> only reads it.
+__device__ __forceinline__ uint32_t draw_byte(const Params& p, uint32_t c0, uint32_t t_lo, uint32_t t_hi)
 {
     uint32_t a0, a1, a2, a3, b0, b1, b2, b3;
-    philox4x32_10(p, c0, p.t_lo, p.t_hi, DOM_BOND, a0, a1, a2, a3);
-    philox4x32_10(p, c0 + 1, p.t_lo, p.t_hi, DOM_BOND, b0, b1, b2, b3);
-    // d: bit 2j = [east draw of site j >= T], bit 2j+1 = [north draw >= T]: the last draw first, it ends up in bit 7
-    uint32_t d = 0;
+    philox4x32_10(p, c0, t_lo, t_hi, DOM_BOND, a0, a1, a2, a3);
+    philox4x32_10(p, c0 + 1, t_lo, t_hi, DOM_BOND, b0, b1, b2, b3);
+    uint32_t d = 0;                                      // the last draw first, it ends up in bit 7
     shift_in_ge(d, b3, p.negT); shift_in_ge(d, b2, p.negT); shift_in_ge(d, b1, p.negT); shift_in_ge(d, b0, p.negT);
     shift_in_ge(d, a3, p.negT); shift_in_ge(d, a2, p.negT); shift_in_ge(d, a1, p.negT); shift_in_ge(d, a0, p.negT);
+    return d;
+}
+
+// The lane's bond byte for row y: bit 2j = east bond of site j, bit 2j+1 = north bond of site j (the packed-bond
+// format of include/swb200.h), for the 4 sites whose spins are w; e = spins of the east neighbours, n = of the north;
+// d = their draw byte.
+template <bool ISING>
+__device__ __forceinline__ uint32_t bond_byte(const Params& p, uint32_t d, uint32_t w, uint32_t e, uint32_t n)
+{
     uint32_t eq;                                         // bit 8j+1: s_j == s_east, bit 8j+2: s_j == s_north
     if (ISING) {                                         // bytes 0x01 / 0xFF: equal <=> bit 1 (and bit 2) of the xor is 0
         eq = (~(w ^ e) & 0x02020202u) | (~(w ^ n) & 0x04040404u);
@@ -125,15 +133,27 @@ __device__ __forceinline__ uint32_t bond_byte(const Params& p, uint32_t c0, uint
     return __umulhi(eq, 0x82082000u) & ~d & p.dmask;     // 2^31 + 2^25 + 2^19 + 2^13
 }
 
-// ---------------------------------------------------------------------------------------------------- k_scan
-// FROM_BONDS=false: read spins, draw bonds (a1).  FROM_BONDS=true: read packed bonds (sw_label).  Writes the provisional
-// labels (`prov`, see label_kernels.cuh) and the edge arrays, and adds the number of active bonds to acc->n_active.
-// FULLW: L is a multiple of TW, every strip has all 32 lanes (no ragged right edge; the predicates fold away).
-template <bool FROM_BONDS, bool ISING, bool FULLW>
-__global__ void __launch_bounds__(SCAN_THREADS)
-k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __restrict__ bonds_in, int* prov,
-       int* __restrict__ edgeA, int* __restrict__ edgeB, Acc* __restrict__ acc)
+// Draw cache (workspace): one 32-bit word per lane and group of 4 rows of a strip, byte r = draw byte of row 4g + r:
+// word index ((ty * ntx + tx) * (TH / 4) + g) * 32 + lane.  Written by k_final<MODE_SW> for step t+1 (its warp g owns rows
+// 4g..4g+3), read by k_scan<SRC_DRAWS> of the next sweep.
+__device__ __forceinline__ size_t draw_word_index(const Params& p, int tx, int ty, int g, int lane)
 {
+    return ((size_t)(ty * p.ntx + tx) * (TH / 4) + g) * 32 + lane;
+}
+
+// ---------------------------------------------------------------------------------------------------- k_scan
+// SRC_PHILOX: read spins, draw bonds (a1).  SRC_DRAWS: read spins and the draw cache k_final filled one sweep ahead (the
+// same bonds, the Philox work done where the issue slots were idle).  SRC_BONDS: read packed bonds (sw_label).  Writes the
+// provisional labels (`prov`, see label_kernels.cuh) and the edge arrays, and adds the number of active bonds to
+// acc->n_active.  FULLW: L is a multiple of TW, every strip has all 32 lanes (no ragged right edge; the predicates fold away).
+enum { SRC_PHILOX = 0, SRC_BONDS = 1, SRC_DRAWS = 2 };
+template <int SRC, bool ISING, bool FULLW>
+__global__ void __launch_bounds__(SCAN_THREADS)
+k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __restrict__ bonds_in,
+       const uint32_t* __restrict__ draws, int* prov, int* __restrict__ edgeA, int* __restrict__ edgeB,
+       Acc* __restrict__ acc)
+{
+    constexpr bool FROM_BONDS = SRC == SRC_BONDS;
     __shared__ __align__(16) uint16_t s_nm[SCAN_WARPS][TW * TH];
     __shared__ uint32_t s_q[SCAN_WARPS][QCAP];
     __shared__ __align__(16) uint4 s_la[128];
@@ -198,9 +218,15 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
     const uint32_t* const pw_halo = spins_w + row_halo + xws;
     const int dxe = xew - xws;
 
+    uint32_t dw = 0;                                     // draw bytes of the rows 4g..4g+3 (SRC_DRAWS)
+    const uint32_t* pdw = draws + (SRC == SRC_DRAWS ? draw_word_index(p, tx, ty, 0, lane) : 0);
     for (int ly = 0; ly < th_eff; ++ly) {
         uint32_t G = 0;                                  // the lane's bond byte of this row
         if (!FROM_BONDS) {
+            uint32_t d;
+            if (SRC == SRC_DRAWS && (ly & 3) == 0) { dw = *pdw; pdw += 32; }
+            if (SRC == SRC_DRAWS && (ly & 3) < GEN_ROWS) d = __byte_perm(dw, 0u, 0x4440u | (uint32_t)(ly & 3));
+            else d = draw_byte(p, c0, p.t_lo, p.t_hi);
             uint32_t w3 = 0, h3 = 0;                     // prefetch row y+3 (the last one is the north halo row)
             if (ly + 3 <= th_eff) {
                 const uint32_t* const q3 = ly + 3 < th_eff ? pw : pw_halo;
@@ -211,7 +237,7 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
             uint32_t wnext = __shfl_down_sync(FULLM, w0, 1);
             if (is_last) wnext = h0;
             const uint32_t east = __funnelshift_r(w0, wnext, 8);
-            G = bond_byte<ISING>(p, c0, w0, east, w1);
+            G = bond_byte<ISING>(p, d, w0, east, w1);
             c0 += (uint32_t)L >> 1;
             w0 = w1; w1 = w2; w2 = w3; h0 = h1; h1 = h2; h2 = h3;
         } else if (colv) {
@@ -343,7 +369,8 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
         if (colv) nact += __popc(eastm);                 // my east bonds into the next lane / out of the strip, all rows
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) nact += __shfl_xor_sync(FULLM, nact, o);
-        if (lane == 0 && nact) atomicAdd(&acc->n_active, (unsigned long long)nact);
+        if (lane == 0 && nact)
+            atomicAdd(&acc->part[(tx + 5 * ty) & (ACC_PARTS - 1)].n_active, (unsigned long long)nact);
     }
 }
 

@@ -32,6 +32,10 @@ struct sw_handle {
     int32_t*  d_edgeA;             // (ntx+nty)*L: strip-local roots of last columns / last rows (-1: bond inactive)
     int32_t*  d_edgeB;             // (ntx+nty)*L: strip-local roots of first columns / first rows
     int32_t*  d_size;              // N int32
+    uint32_t* d_draws;             // draw cache: ntx*nty*TH/4*32 words (scan_kernel.cuh)
+    bool      draws_valid;         // the cache holds the draws of step draws_t for threshold draws_T
+    uint64_t  draws_t;
+    uint32_t  draws_T;
     bool      bound;
     const int32_t* last_labels;    // labels buffer written by the LAST sweep / step / sw_label (NULL: none since bind)
     uint64_t  launches;
@@ -47,7 +51,7 @@ namespace {
 constexpr size_t ALIGN = 256;
 inline size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
-struct WorkLayout { size_t acc, wolff, edgeA, edgeB, size, total; };
+struct WorkLayout { size_t acc, wolff, edgeA, edgeB, draws, size, total; };
 
 WorkLayout work_layout(int32_t L)
 {
@@ -58,7 +62,8 @@ WorkLayout work_layout(int32_t L)
     w.wolff = align_up(sizeof(Acc));
     w.edgeA = w.wolff + align_up(sizeof(unsigned long long) * WOLFF_RING);
     w.edgeB = w.edgeA + align_up((ntx + nty) * (size_t)L * sizeof(int32_t));
-    w.size = w.edgeB + align_up((ntx + nty) * (size_t)L * sizeof(int32_t));
+    w.draws = w.edgeB + align_up((ntx + nty) * (size_t)L * sizeof(int32_t));
+    w.size = w.draws + align_up(ntx * nty * (size_t)(TH / 4) * 32 * sizeof(uint32_t));
     w.total = w.size + align_up(N * sizeof(int32_t));
     return w;
 }
@@ -106,6 +111,8 @@ Params params_at(const sw_handle* h, uint64_t t)
     p.dmask = h->T ? 0xFFu : 0u;
     p.t_lo = (uint32_t)(t & 0xFFFFFFFFu);
     p.t_hi = (uint32_t)(t >> 32);
+    p.u_lo = (uint32_t)((t + 1) & 0xFFFFFFFFu);
+    p.u_hi = (uint32_t)((t + 1) >> 32);
     return p;
 }
 
@@ -126,15 +133,21 @@ inline int grid_for(int64_t n, int block) { return (int)((n + block - 1) / block
 inline int grid_capped(int64_t n, int block, int cap) { int g = grid_for(n, block); return g < cap ? (g < 1 ? 1 : g) : cap; }
 
 // labelling of the bond graph of step t (or of packed bonds): k_scan -> k_seam; k_final resolves the rest
-template <bool FROM_BONDS>
+// SRC_PHILOX falls through to SRC_DRAWS when the draw cache holds the draws of step t for the current threshold
+template <int SRC>
 int launch_label_front(sw_handle* h, const Params& p, const uint8_t* bonds, int32_t* labels, cudaStream_t s)
 {
     SW_PROF(h, 0, s);
     const dim3 grid((p.ntx + SCAN_WARPS - 1) / SCAN_WARPS, p.nty);
-    const bool ising = FROM_BONDS || p.q == 2, fullw = (p.L % TW) == 0;
-    auto kern = ising ? (fullw ? k_scan<FROM_BONDS, true, true> : k_scan<FROM_BONDS, true, false>)
-                      : (fullw ? k_scan<false, false, true> : k_scan<false, false, false>);
-    kern<<<grid, SCAN_THREADS, 0, s>>>(p, h->d_spins, bonds, labels, h->d_edgeA, h->d_edgeB, h->d_acc);
+    const bool ising = SRC == SRC_BONDS || p.q == 2, fullw = (p.L % TW) == 0;
+    const uint64_t t = ((uint64_t)p.t_hi << 32) | p.t_lo;
+    const bool cached = SRC == SRC_PHILOX && h->draws_valid && h->draws_t == t && h->draws_T == h->T;
+    auto kern = SRC == SRC_BONDS ? (fullw ? k_scan<SRC_BONDS, true, true> : k_scan<SRC_BONDS, true, false>)
+              : cached ? (ising ? (fullw ? k_scan<SRC_DRAWS, true, true> : k_scan<SRC_DRAWS, true, false>)
+                                : (fullw ? k_scan<SRC_DRAWS, false, true> : k_scan<SRC_DRAWS, false, false>))
+                       : (ising ? (fullw ? k_scan<SRC_PHILOX, true, true> : k_scan<SRC_PHILOX, true, false>)
+                                : (fullw ? k_scan<SRC_PHILOX, false, true> : k_scan<SRC_PHILOX, false, false>));
+    kern<<<grid, SCAN_THREADS, 0, s>>>(p, h->d_spins, bonds, h->d_draws, labels, h->d_edgeA, h->d_edgeB, h->d_acc);
     SW_LAUNCHED(h, "k_scan");
     SW_PROF(h, 1, s);
     const int nseam = (p.ntx + p.nty) * p.L;
@@ -146,8 +159,8 @@ int launch_label_front(sw_handle* h, const Params& p, const uint8_t* bonds, int3
 
 int zero_sweep_counters(sw_handle* h, cudaStream_t s)
 {
-    // n_active and n_clusters are adjacent at the start of Acc
-    SW_CUDA(h, cudaMemsetAsync(h->d_acc, 0, 2 * sizeof(unsigned long long), s));
+    // the per-sweep counters (n_active, n_clusters) are the parts at the start of Acc
+    SW_CUDA(h, cudaMemsetAsync(h->d_acc, 0, sizeof(AccPart) * ACC_PARTS, s));
     return SW_OK;
 }
 
@@ -258,6 +271,8 @@ int sw_bind(sw_handle* h, void* d_spins, int32_t* d_labels, uint8_t* d_bonds, vo
     h->d_edgeA = (int32_t*)(h->d_work + w.edgeA);
     h->d_edgeB = (int32_t*)(h->d_work + w.edgeB);
     h->d_size = (int32_t*)(h->d_work + w.size);
+    h->d_draws = (uint32_t*)(h->d_work + w.draws);
+    h->draws_valid = false;
     h->bound = false;
     h->last_labels = nullptr;
     SW_CUDA(h, cudaMemsetAsync(h->d_work, 0, w.edgeA, (cudaStream_t)stream));
@@ -290,10 +305,17 @@ int sw_sweep(sw_handle* h, int64_t n, void* stream)
         const Params p = params_at(h, h->t);
         int rc = zero_sweep_counters(h, s);
         if (rc) return rc;
-        rc = launch_label_front<false>(h, p, nullptr, h->d_labels, s);
+        rc = launch_label_front<SRC_PHILOX>(h, p, nullptr, h->d_labels, s);
         if (rc) return rc;
-        k_final<MODE_SW><<<dim3(p.ntx, p.nty), FIN_THREADS, 0, s>>>(p, h->d_labels, h->d_spins, h->d_acc, nullptr);
+        // the flatten + flip pass also draws the bonds of step t+1 (draw cache): the next sweep's k_scan only reads them
+        {
+            const bool full = (p.L % TW) == 0 && (p.L % TH) == 0, q2 = p.q == 2;
+            auto fin = full ? (q2 ? k_final<MODE_SW, GEN_ROWS, true, true> : k_final<MODE_SW, GEN_ROWS, true, false>)
+                            : (q2 ? k_final<MODE_SW, GEN_ROWS, false, true> : k_final<MODE_SW, GEN_ROWS, false, false>);
+            fin<<<dim3(p.ntx, p.nty), FIN_THREADS, 0, s>>>(p, h->d_labels, h->d_spins, h->d_acc, nullptr, h->d_draws);
+        }
         SW_LAUNCHED(h, "k_final<SW>");
+        h->draws_valid = GEN_ROWS > 0; h->draws_t = h->t + 1; h->draws_T = h->T;
         SW_PROF(h, 3, s);
         if (h->prof_on && h->prof_n < PROF_MAX) ++h->prof_n;
         ++h->t;
@@ -327,9 +349,12 @@ int sw_label(sw_handle* h, const uint8_t* d_bonds_in, int32_t* d_labels_out, voi
     const Params p = params_at(h, h->t);
     int rc = zero_sweep_counters(h, s);
     if (rc) return rc;
-    rc = launch_label_front<true>(h, p, bonds, labels, s);
+    rc = launch_label_front<SRC_BONDS>(h, p, bonds, labels, s);
     if (rc) return rc;
-    k_final<MODE_LABEL><<<dim3(p.ntx, p.nty), FIN_THREADS, 0, s>>>(p, labels, nullptr, h->d_acc, nullptr);
+    if ((p.L % TW) == 0 && (p.L % TH) == 0)
+        k_final<MODE_LABEL, 0, true, true><<<dim3(p.ntx, p.nty), FIN_THREADS, 0, s>>>(p, labels, nullptr, h->d_acc, nullptr, nullptr);
+    else
+        k_final<MODE_LABEL, 0, false, true><<<dim3(p.ntx, p.nty), FIN_THREADS, 0, s>>>(p, labels, nullptr, h->d_acc, nullptr, nullptr);
     SW_LAUNCHED(h, "k_final<LABEL>");
     SW_PROF(h, 3, s);
     if (h->prof_on && h->prof_n < PROF_MAX) ++h->prof_n;
@@ -382,10 +407,14 @@ int wolff_step(sw_handle* h, int64_t n, int64_t* h_sizes, void* stream)
             const Params p = params_at(h, h->t);
             int rc = zero_sweep_counters(h, s);
             if (rc) return rc;
-            rc = launch_label_front<false>(h, p, nullptr, h->d_labels, s);
+            rc = launch_label_front<SRC_PHILOX>(h, p, nullptr, h->d_labels, s);
             if (rc) return rc;
-            k_final<MODE_WOLFF><<<dim3(p.ntx, p.nty), FIN_THREADS, 0, s>>>(p, h->d_labels, h->d_spins, h->d_acc,
-                                                                         h->d_wolff + k);
+            if ((p.L % TW) == 0 && (p.L % TH) == 0)
+                k_final<MODE_WOLFF, 0, true, true><<<dim3(p.ntx, p.nty), FIN_THREADS, 0, s>>>(p, h->d_labels, h->d_spins,
+                                                                                            h->d_acc, h->d_wolff + k, nullptr);
+            else
+                k_final<MODE_WOLFF, 0, false, true><<<dim3(p.ntx, p.nty), FIN_THREADS, 0, s>>>(p, h->d_labels, h->d_spins,
+                                                                                             h->d_acc, h->d_wolff + k, nullptr);
             SW_LAUNCHED(h, "k_final<WOLFF>");
             SW_PROF(h, 3, s);
             if (h->prof_on && h->prof_n < PROF_MAX) ++h->prof_n;
@@ -439,8 +468,10 @@ int sw_observables_ex(sw_handle* h, sw_obs* h_out, int flags, void* stream)
         }
     }
     if (h->last_labels) {                                // counted by the labelling itself: free
-        h_out->n_clusters = (int64_t)a.n_clusters;
-        h_out->n_active_bonds = (int64_t)a.n_active;
+        for (int k = 0; k < ACC_PARTS; ++k) {
+            h_out->n_clusters += (int64_t)a.part[k].n_clusters;
+            h_out->n_active_bonds += (int64_t)a.part[k].n_active;
+        }
     }
     if (clusters) {
         h_out->max_cluster = (int64_t)a.cs_max;
