@@ -35,7 +35,7 @@ __device__ __forceinline__ int strip_gidx(int base, int L, int l) { return base 
 // Private to one warp.
 //
 // find with path halving.  Plain loads/stores: halving rewrites non-root entries with an ancestor (concurrent lanes may
-// interleave, every value written is an ancestor); roots change only in phase 2 of unite_batch.
+// interleave, every value written is an ancestor); roots change only in phase 2 of unite_batch (scan_kernel.cuh).
 __device__ __forceinline__ int nm_find(volatile uint16_t* nm, int x)
 {
     int p = nm[x];
@@ -58,32 +58,6 @@ __device__ __forceinline__ void nm_root4(const volatile uint16_t* nm, int& a, in
         pa = nm[a]; pb = nm[b]; pc = nm[c]; pd = nm[d];
     }
 }
-
-// Unite one queued pair of names per lane (pair = a << 16 | b), hooking the larger root under the smaller and writing
-// every hook through to `prov`.  3-phase protocol, no atomics (the forest belongs to this warp): (1) all lanes find
-// roots -- nobody hooks, so a root stays a root; (2) hook with a plain store -- lanes hooking the same root collide, one
-// store wins; (3) re-read: losers retry from the new roots.
-__device__ __forceinline__ void unite_batch(volatile uint16_t* nm, bool have, uint32_t pair, int* prov, int base, int L)
-{
-    int ua = (int)(pair >> 16), ub = (int)(pair & 0xFFFFu);
-    while (__any_sync(FULLM, have)) {
-        if (have) {
-            ua = nm_find(nm, ua);
-            ub = nm_find(nm, ub);
-            if (ua == ub) have = false;
-            else if (ua < ub) { const int t = ua; ua = ub; ub = t; }
-        }
-        __syncwarp();
-        if (have) nm[ua] = (uint16_t)ub;
-        __syncwarp();
-        if (have && nm[ua] == ub) {
-            prov[strip_gidx(base, L, ua)] = REF | HOOK | ub;
-            have = false;
-        }
-    }
-}
-
-constexpr int QCAP = 32 + TW;                            // < 32 pairs carried over + at most one new pair per site of a row
 
 // Edge arrays (workspace): for every site on the edge of a strip the global index of its strip-local root.
 //   edgeA = [ rootE (ntx * L) | rootN (nty * L) ] : last column of strip column tc at row y -> [tc * L + y], last row of

@@ -1,99 +1,170 @@
 // scan_kernel.cuh -- k_scan: bond activation (P:53 step 1, Eq. 7) fused with strip-local labelling.
-// Included by label_kernels.cuh (uses its forest helpers nm_find / nm_root4 / unite_batch and the `prov` encoding).
+// Included by label_kernels.cuh (uses its forest helpers nm_find / nm_root4 and the `prov` encoding).
 //
-// One warp per TW x TH strip, lane -> 4 consecutive columns, rows in sequence.  A "node" is a horizontal run (inside the
-// strip) that has no active north bond from the row above; it is named by its first site.  Every other run adopts the
-// name carried by its leftmost contact with the row above, so every name is a node.  When a run has further contacts
-// whose names differ from the adopted one, the pair of names is queued; queued pairs are united 32 at a time (all lanes
-// busy) in the strip's forest.  Names never depend on the forest, so the row loop has no divergent part.
+// One warp per TW x TH strip, lane -> 4 consecutive columns, rows in sequence.  A "node" is a site that names a run: the
+// first site of a part of a horizontal run (the part inside one lane, or inside two neighbouring lanes) that has no active
+// north bond from the row above.  Every other site adopts the name carried by the leftmost contact of its part with the row
+// above, so every name is a node.  Wherever two names meet that are not known to be equal -- a contact whose carried name
+// differs from the adopted one, or a run that continues from the left lane into a fully bonded lane -- a flag bit is set;
+// the flagged site positions are collected every 8 rows and their names united, 32 pairs at a time (all lanes busy), in
+// the strip's forest.  Names never depend on the forest, so the row loop has no divergent part.
 //
-// Names are strip-local site indices (< TW*TH = 4096) kept as 16-bit halves, two per register: P01/P23 = names carried
-// by the 4 sites of the previous row, l01/l23 = names of this row.  Which name a site takes is a function of 7 bits --
-// the lane's 3 inner east bonds and the 4 north bonds from the row above -- so it comes from a 128-entry table of byte
-// permutation selectors (PRMT): 4 permutes name the 4 sites, 2 more (selectors from a second table, indexed by the 4
-// east bonds and the link from the previous lane) substitute the names of runs that cross lane boundaries.
+// The kernel is bound by the integer ALU pipe (LOP3, PRMT, ISETP, SEL, SHF: one warp instruction per 2 clocks per
+// sub-partition; measured, profiles/r02_README.md), so the row loop is written to keep work OFF that pipe:
+//   - names are strip-local site indices (< TW*TH = 4096) kept as 16-bit halves, two per register (P01/P23 = names
+//     carried by the 4 sites of the previous row, l01/l23 = names of this row); which name a site takes inside its lane is
+//     a function of 8 bits -- the lane's 4 east bonds and the 4 north bonds from the row above -- so it comes from a
+//     256-entry table of byte-permutation selectors: 4 PRMT name the 4 sites;
+//   - a run that crosses into the next lane is resolved between the two neighbours only: two shuffles carry the suffix name
+//     of the left lane and the prefix name of the right lane plus flag bits; masks from the same table entry decide with one
+//     LOP3 each whether the lane's prefix / suffix part takes the neighbour's name (predicated PRMTs, selectors from a second
+//     small table).  No ballots, no bit scans.  A fully bonded lane keeps its own name and flags the link instead;
+//   - "is this half-word non-zero" for the 4 mismatch tests is an add that carries out of the 12-bit name, on the
+//     multiply-add pipe; the 4 carries are gathered with a multiply-high; flag words are accumulated with multiply-adds.
 #pragma once
 #include "common.cuh"
 
 namespace swb {
+
+static_assert(TW * TH <= 4096, "names are 12-bit strip-local site indices");
+
+// ---------------------------------------------------------------------------------------------------- host/device helpers
+// PRMT reads the 4 selector nibbles of s[15:0] only (every nibble here is < 8: plain byte select); the upper half of a
+// selector word is free for other table data.  The host versions serve tests/host/scan_row_check.cu.
+#define SWB_HD __host__ __device__ __forceinline__
+SWB_HD uint32_t prmt(uint32_t a, uint32_t b, uint32_t s)
+{
+#ifdef __CUDA_ARCH__
+    uint32_t d;
+    asm("prmt.b32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(s));
+    return d;
+#else
+    const uint64_t ab = ((uint64_t)b << 32) | a;
+    uint32_t d = 0;
+    for (int i = 0; i < 4; ++i) d |= (uint32_t)((ab >> (8 * ((s >> (4 * i)) & 7))) & 0xFF) << (8 * i);
+    return d;
+#endif
+}
+SWB_HD uint32_t mulhi_u32(uint32_t a, uint32_t b)
+{
+#ifdef __CUDA_ARCH__
+    return __umulhi(a, b);
+#else
+    return (uint32_t)(((uint64_t)a * b) >> 32);
+#endif
+}
 
 // ---------------------------------------------------------------------------------------------------- tables
 // A half h in [0,4) of a register pair (a, b) seen by PRMT: 0 = a.lo, 1 = a.hi, 2 = b.lo, 3 = b.hi.
 constexpr uint32_t lut_half(int h) { return (uint32_t)(((2 * h + 1) << 4) | (2 * h)); }
 constexpr uint32_t lut_sel(int hlo, int hhi) { return lut_half(hlo) | (lut_half(hhi) << 8); }
 
+// Flag bits in the upper halves of the table words (the lower halves are PRMT selectors)
+constexpr uint32_t F_LK = 1u << 16;      // a[0]: my east bond into the next lane is active (sent to the right neighbour)
+constexpr uint32_t F_LC = 1u << 17;      // a[0]: ... and my suffix part has a contact
+constexpr uint32_t F_CP = 1u << 20;      // a[1]: my prefix part has a contact (sent to the left neighbour)
+                                         // a[1] bits 16,17: link-flag masks against the left neighbour's F_LK, F_LC
+                                         // a[2] bits 16,17: prefix-substitution masks against F_LK, F_LC; bit 20: suffix-
+                                         //                  substitution mask against the right neighbour's F_CP
+                                         // a[3] bits 16..19: north contacts of sites 0..3
+
 struct ScanLut {
-    uint32_t a[128][4];    // index: bits 0,2,4 = E0,E1,E2 (east bonds site j -> j+1 of this row), bits 1,3,5,6 = north bonds
-                           // from the previous row into sites 0..3 (the bond byte with bit 7 moved to bit 6)
-    uint32_t b[128];       // index: bits 0,2,4,6 = E0..E3 (E3 = east bond into the next lane), bit 1 = EL (link from the
-                           // previous lane)
+    uint32_t a[256][4];    // index: bit 2j = E_j (east bond site j -> j+1, E_3 into the next lane), bit 2j+1 = north bond from
+                           // the previous row into site j: (bond byte of this row & 0x55) | (bond byte of the previous & 0xAA)
+    uint32_t b[22][4];     // index: bond byte & 0x15 (E_0, E_1, E_2): which sites belong to the prefix / suffix part
 };
 
 constexpr ScanLut make_scan_lut()
 {
     ScanLut t{};
-    for (int i = 0; i < 128; ++i) {
-        const bool E0 = i & 1, E1 = i & 4, E2 = i & 16;
-        const int np = ((i >> 1) & 1) | (((i >> 3) & 1) << 1) | (((i >> 5) & 1) << 2) | (((i >> 6) & 1) << 3);
-        int s[4] = {0, 0, 0, 0};                         // first site of each site's segment (run inside the lane)
+    for (int i = 0; i < 256; ++i) {
+        const bool E0 = i & 1, E1 = i & 4, E2 = i & 16, E3 = i & 64;
+        const int np = ((i >> 1) & 1) | (((i >> 3) & 1) << 1) | (((i >> 5) & 1) << 2) | (((i >> 7) & 1) << 3);
+        int s[4] = {0, 0, 0, 0};                         // first site of each site's part (run inside the lane)
         s[1] = E0 ? 0 : 1;
         s[2] = E1 ? s[1] : 2;
         s[3] = E2 ? s[2] : 3;
-        int lc[4] = {-1, -1, -1, -1};                    // leftmost contact of the segment, -1: none
+        int lc[4] = {-1, -1, -1, -1};                    // leftmost contact of the part, -1: none
         for (int j = 0; j < 4; ++j)
             for (int k = 3; k >= 0; --k)
                 if (s[k] == s[j] && ((np >> k) & 1)) lc[j] = k;
         // X = prmt(P01, P23, selX): the contact names that sites 0 and 1 may take
         const uint32_t selX = lut_sel(lc[0] < 0 ? 0 : lc[0], lc[1] < 0 ? 0 : lc[1]);
-        // l01 = prmt(X, NEW01, selL01): contact name, else a new node named by the segment's first site
+        // l01 = prmt(X, NEW01, selL01): contact name, else a new node named by the part's first site
         const uint32_t selL01 = lut_sel(lc[0] < 0 ? 2 : 0, lc[1] < 0 ? 2 + s[1] : 1);
-        // W = prmt(P23, NEW23, selW): names of sites 2 / 3 if they start a segment (s == own index)
+        // W = prmt(P23, NEW23, selW): names of sites 2 / 3 if they start a part (s == own index)
         const int wlo = s[2] != 2 ? 0 : (lc[2] < 0 ? 2 : lc[2] - 2);
         const int whi = (np & 8) ? 1 : 3;
         const uint32_t selW = lut_sel(wlo, whi);
-        // l23 = prmt(W, l01, selL23): a site whose segment starts at 0 or 1 takes l1
+        // l23 = prmt(W, l01, selL23): a site whose part starts at 0 or 1 takes l1
         const uint32_t selL23 = lut_sel(s[2] == 2 ? 0 : 3, s[3] == 3 ? 1 : (s[3] == 2 ? 0 : 3));
-        // masks of the sites that have a contact: prmt(0x0000FFFF, x, sel) -> 0xFFFF in the halves with a contact
-        const uint32_t m01 = lut_sel((np & 1) ? 0 : 1, (np & 2) ? 0 : 1);
-        const uint32_t m23 = lut_sel((np & 4) ? 0 : 1, (np & 8) ? 0 : 1);
-        int cnt = 0;                                     // active bonds in the pattern
-        for (int k = 0; k < 7; ++k) cnt += (i >> k) & 1;
-        t.a[i][0] = selX | (selL01 << 16);
-        t.a[i][1] = selW | (selL23 << 16);
-        t.a[i][2] = m01 | (m23 << 16);
-        // bit 0: the suffix segment (site 3's) has a contact; bit 1: the prefix segment (site 0's) has one; top: count
-        t.a[i][3] = (lc[3] >= 0 ? 1u : 0u) | (lc[0] >= 0 ? 2u : 0u) | ((uint32_t)cnt << 28);
+        const bool full = E0 && E1 && E2, cp = lc[0] >= 0, cs = lc[3] >= 0;
+        t.a[i][0] = selX | (E3 ? F_LK : 0u) | (E3 && cs ? F_LC : 0u);
+        // link flag (fully bonded lanes only): the run continues from the left lane and this lane keeps its own name --
+        // unless the left part has no contact and this lane has one (then the left part takes this lane's name)
+        t.a[i][1] = selL01 | (cp ? F_CP : 0u) | (full && !cp ? F_LK : 0u) | (full ? F_LC : 0u);
+        // the prefix part takes the left suffix name if the link is active and (the left part has a contact or mine has
+        // none); the suffix part takes the right prefix name if my link is active, mine has no contact and the right has one
+        t.a[i][2] = selW | (!full && !cp ? F_LK : 0u) | (!full ? F_LC : 0u) | (E3 && !cs ? F_CP : 0u);
+        t.a[i][3] = selL23 | ((uint32_t)np << 16);
     }
-    for (int i = 0; i < 128; ++i) {
-        const bool E0 = i & 1, E1 = i & 4, E2 = i & 16, E3 = i & 64, EL = i & 2;
+    for (int i = 0; i < 22; ++i) {
+        const bool E0 = i & 1, E1 = i & 4, E2 = i & 16;
         int s[4] = {0, 0, 0, 0};
         s[1] = E0 ? 0 : 1;
         s[2] = E1 ? s[1] : 2;
         s[3] = E2 ? s[2] : 3;
-        const bool full = E0 && E1 && E2;
-        const bool useP = EL && !full, useS = E3 || (full && EL);
-        int h[4] = {0, 1, 0, 1};                         // l01' = prmt(l01, RP|RS<<16, .), l23' = prmt(l23, RP|RS<<16, .)
-        for (int j = 0; j < 4; ++j) {
-            if (useS && s[j] == s[3]) h[j] = 3;          // in the run that leaves the lane to the right: RS
-            else if (useP && s[j] == 0) h[j] = 2;        // in the run that enters from the left: RP
-        }
-        t.b[i] = lut_sel(h[0], h[1]) | (lut_sel(h[2], h[3]) << 16);
+        // l' = prmt(l, nb, sel): own halves 0, 1; the neighbour's name is the low half of nb = half 2
+        t.b[i][0] = lut_sel(2, s[1] == 0 ? 2 : 1);                              // prefix part, sites 0 1
+        t.b[i][1] = lut_sel(s[2] == 0 ? 2 : 0, s[3] == 0 ? 2 : 1);              // prefix part, sites 2 3
+        t.b[i][2] = lut_sel(s[0] == s[3] ? 2 : 0, s[1] == s[3] ? 2 : 1);        // suffix part, sites 0 1
+        t.b[i][3] = lut_sel(s[2] == s[3] ? 2 : 0, 2);                           // suffix part, sites 2 3
     }
     return t;
 }
 
-__device__ const ScanLut d_scan_lut = make_scan_lut();
-
-// ---------------------------------------------------------------------------------------------------- helpers
-// PRMT reads the 4 selector nibbles of s[15:0] only (every nibble here is < 8: plain byte select); __byte_perm would
-// spend an extra instruction masking the selector.
-__device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t s)
+// ---------------------------------------------------------------------------------------------------- one row of one lane
+// Part 1: names from the lane's own bonds and contacts, and the two messages to the neighbouring lanes:
+//   to the right: suffix name | F_LK, F_LC      to the left: prefix name | F_CP
+SWB_HD void row_local(const uint32_t A[4], uint32_t P01, uint32_t P23, uint32_t NEW01, uint32_t NEW23,
+                      uint32_t& l01, uint32_t& l23, uint32_t& to_right, uint32_t& to_left)
 {
-    uint32_t d;
-    asm("prmt.b32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(s));
-    return d;
+    const uint32_t X = prmt(P01, P23, A[0]);
+    l01 = prmt(X, NEW01, A[1]);
+    const uint32_t W = prmt(P23, NEW23, A[2]);
+    l23 = prmt(W, l01, A[3]);
+    to_right = prmt(l23, A[0], 0x7632);                  // l3 | upper half of A[0]
+    to_left = prmt(l01, A[1], 0x7610);                   // l0 | upper half of A[1]
 }
 
+// Part 2: substitute the neighbours' names where the table masks say so; returns the link flag (0 / non-zero in bits
+// 16,17).  left_ok = F_LK | F_LC, or 0 for the first lane of the strip (no left neighbour).
+SWB_HD uint32_t row_final(const uint32_t A[4], const uint32_t B[4], uint32_t from_left, uint32_t from_right,
+                          uint32_t left_ok, uint32_t& l01, uint32_t& l23)
+{
+    const bool subP = (from_left & A[2] & left_ok) != 0u;
+    const bool subS = (from_right & A[2] & F_CP) != 0u;
+    if (subP) { l01 = prmt(l01, from_left, B[0]); l23 = prmt(l23, from_left, B[1]); }
+    if (subS) { l01 = prmt(l01, from_right, B[2]); l23 = prmt(l23, from_right, B[3]); }
+    return from_left & A[1] & left_ok;
+}
+
+// The 4 mismatch flags of the row in bits 16..19: site j carries a contact (north bond from the row above) whose name P_j
+// differs from the name l_j it has taken.  Names are < 4096: x + 0x0FFF carries into bit 12 iff x != 0.
+SWB_HD uint32_t row_mismatch(const uint32_t A[4], uint32_t P01, uint32_t P23, uint32_t l01, uint32_t l23)
+{
+    const uint32_t t01 = (P01 ^ l01) + 0x0FFF0FFFu;                      // bits 12, 28: sites 0, 1
+    const uint32_t t23 = (P23 ^ l23) * 4u + 0x3FFC3FFCu;                 // bits 14, 30: sites 2, 3
+    const uint32_t r = (t01 & 0x10001000u) | (t23 & 0x40004000u);
+    // gather bits 12, 28, 14, 30 into bits 0, 1, 2, 3 of the high word: 2^20 moves 12 -> 0 and 14 -> 2, 2^5 moves 28 -> 1 and
+    // 30 -> 3; the cross terms land on bits 16, 18 (shifted out below) or in the low word
+    const uint32_t nib = mulhi_u32(r, (1u << 20) | (1u << 5));
+    return (nib << 16) & A[3];
+}
+
+__device__ const ScanLut d_scan_lut = make_scan_lut();
+
+// ---------------------------------------------------------------------------------------------------- device helpers
 // d <- 2 d + [u >= T] for T != 0: the carry of u + (2^32 - T) shifted into d.  An add with carry-out (ALU pipe) and an
 // add with carry-in (ptxas issues it as IMAD.X on the multiply-add pipe): no compare, select or shift.
 __device__ __forceinline__ void shift_in_ge(uint32_t& d, uint32_t u, uint32_t negT)
@@ -101,9 +172,23 @@ __device__ __forceinline__ void shift_in_ge(uint32_t& d, uint32_t u, uint32_t ne
     asm("{\n\t.reg .u32 t;\n\tadd.cc.u32 t, %1, %2;\n\taddc.u32 %0, %0, %0;\n\t}" : "+r"(d) : "r"(u), "r"(negT));
 }
 
+// a * b + c on the multiply-add pipe (the compiler would turn a multiply by a power of two into an ALU shift)
+__device__ __forceinline__ uint32_t mad_lo(uint32_t a, uint32_t b, uint32_t c)
+{
+    uint32_t d;
+    asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+    return d;
+}
+__device__ __forceinline__ uint32_t mad_hi(uint32_t a, uint32_t b, uint32_t c)
+{
+    uint32_t d;
+    asm("mad.hi.u32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+    return d;
+}
+
 // Draw byte of the 4 sites whose first pair has Philox counter c0, at step (t_lo, t_hi): bit 2j = [east draw of site j
 // >= T], bit 2j+1 = [north draw >= T] (S:8c.3: u(i,d,t) = PHILOX(seed; i>>1, t, BOND)[2(i&1)+d]).  A pure function of
-// (seed, t, site, T): k_final computes it one sweep ahead (draw cache, see k_final) and k_scan<SRC_DRAWS> only reads it.
+// (seed, t, site, T): k_final can compute it one sweep ahead (draw cache, see k_final) and k_scan<SRC_DRAWS> only reads it.
 __device__ __forceinline__ uint32_t draw_byte(const Params& p, uint32_t c0, uint32_t t_lo, uint32_t t_hi)
 {
     uint32_t a0, a1, a2, a3, b0, b1, b2, b3;
@@ -141,11 +226,73 @@ __device__ __forceinline__ size_t draw_word_index(const Params& p, int tx, int t
     return ((size_t)(ty * p.ntx + tx) * (TH / 4) + g) * 32 + lane;
 }
 
+// ---------------------------------------------------------------------------------------------------- unions
+// Queue entries: bits 0..11 = strip-local position p of a flagged site, QEAST set: unite the names of p and of its west
+// neighbour p - 1 (link flag), else of p and of the site above it, p - TW (mismatch flag).  Names are read back from the
+// forest array: entry of a site = the name it took (a node) or, for a node, its parent.
+constexpr uint32_t QEAST = 0x8000u;
+constexpr int QCAP = 64;                                 // < 32 entries carried over + at most 32 new ones per round
+
+// Unite one queued pair per lane, hooking the larger root under the smaller and writing every hook through to `prov`.
+// 3-phase protocol, no atomics (the forest belongs to this warp): (1) all lanes find roots -- nobody hooks, so a root stays
+// a root; (2) hook with a plain store -- lanes hooking the same root collide, one store wins; (3) re-read: losers retry
+// from the new roots.
+__device__ __forceinline__ void unite_batch(volatile uint16_t* nm, bool have, uint32_t code, int* prov, int base, int L)
+{
+    int ua = 0, ub = 0;
+    if (have) {
+        const int pos = (int)(code & 0x0FFFu);
+        ua = nm[pos];
+        ub = nm[pos - ((code & QEAST) ? 1 : TW)];
+    }
+    while (__any_sync(FULLM, have)) {
+        if (have) {
+            ua = nm_find(nm, ua);
+            ub = nm_find(nm, ub);
+            if (ua == ub) have = false;
+            else if (ua < ub) { const int t = ua; ua = ub; ub = t; }
+        }
+        __syncwarp();
+        if (have) nm[ua] = (uint16_t)ub;
+        __syncwarp();
+        if (have && nm[ua] == ub) {
+            prov[strip_gidx(base, L, ua)] = REF | HOOK | ub;
+            have = false;
+        }
+    }
+}
+
+// Collect the flagged sites of a lane's flag word into the warp's queue and unite them 32 at a time.  Bit b of `flags`
+// stands for the strip-local position pos0 - (b >> sh) * TW + (b & ((1 << sh) - 1)) (sh = 2: 4 mismatch flags per row, the
+// newest row in bits 0..3; sh = 0: one link flag per row) | tag.  Every round each lane that still has a flag appends one.
+__device__ __forceinline__ void drain_flags(uint32_t flags, int sh, int pos0, uint32_t tag, volatile uint16_t* q, int& qn,
+                                            volatile uint16_t* nm, int* prov, int base, int L, int lane, unsigned lt)
+{
+    while (true) {
+        const bool has = flags != 0u;
+        const unsigned Bm = __ballot_sync(FULLM, has);
+        if (Bm == 0u) break;
+        if (has) {
+            const int b = 31 - __clz(flags);
+            flags ^= 1u << b;
+            const int pos = pos0 - ((b >> sh) << TW_LOG) + (b & ((1 << sh) - 1));
+            q[qn + __popc(Bm & lt)] = (uint16_t)((uint32_t)pos | tag);
+        }
+        qn += __popc(Bm);
+        if (qn >= 32) {
+            __syncwarp();                                // queue entries and forest rows visible to the whole warp
+            qn -= 32;
+            unite_batch(nm, true, q[qn + lane], prov, base, L);
+            __syncwarp();                                // queue slots read before they are overwritten
+        }
+    }
+}
+
 // ---------------------------------------------------------------------------------------------------- k_scan
 // SRC_PHILOX: read spins, draw bonds (a1).  SRC_DRAWS: read spins and the draw cache k_final filled one sweep ahead (the
-// same bonds, the Philox work done where the issue slots were idle).  SRC_BONDS: read packed bonds (sw_label).  Writes the
-// provisional labels (`prov`, see label_kernels.cuh) and the edge arrays, and adds the number of active bonds to
-// acc->n_active.  FULLW: L is a multiple of TW, every strip has all 32 lanes (no ragged right edge; the predicates fold away).
+// same bonds, the Philox work done elsewhere).  SRC_BONDS: read packed bonds (sw_label).  Writes the provisional labels
+// (`prov`, see label_kernels.cuh) and the edge arrays, and adds the number of active bonds to the sweep counters.
+// FULLW: L is a multiple of TW, every strip has all 32 lanes (no ragged right edge; the predicates fold away).
 enum { SRC_PHILOX = 0, SRC_BONDS = 1, SRC_DRAWS = 2 };
 template <int SRC, bool ISING, bool FULLW>
 __global__ void __launch_bounds__(SCAN_THREADS)
@@ -155,12 +302,14 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
 {
     constexpr bool FROM_BONDS = SRC == SRC_BONDS;
     __shared__ __align__(16) uint16_t s_nm[SCAN_WARPS][TW * TH];
-    __shared__ uint32_t s_q[SCAN_WARPS][QCAP];
-    __shared__ __align__(16) uint4 s_la[128];
-    __shared__ uint32_t s_lb[128];
-    for (int i = threadIdx.x; i < 128; i += SCAN_THREADS)
+    __shared__ __align__(16) uint4 s_la[256];
+    __shared__ __align__(16) uint4 s_lb[22];
+    __shared__ uint16_t s_q[SCAN_WARPS][QCAP];
+    __shared__ uint8_t s_e3[SCAN_WARPS][TH];             // bond byte of the strip's last lane, row by row (bit 6 leaves the strip)
+    for (int i = threadIdx.x; i < 256; i += SCAN_THREADS)
         s_la[i] = make_uint4(d_scan_lut.a[i][0], d_scan_lut.a[i][1], d_scan_lut.a[i][2], d_scan_lut.a[i][3]);
-    for (int i = threadIdx.x; i < 128; i += SCAN_THREADS) s_lb[i] = d_scan_lut.b[i];
+    for (int i = threadIdx.x; i < 22; i += SCAN_THREADS)
+        s_lb[i] = make_uint4(d_scan_lut.b[i][0], d_scan_lut.b[i][1], d_scan_lut.b[i][2], d_scan_lut.b[i][3]);
     __syncthreads();                                     // the only block-wide barrier
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -168,10 +317,10 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
     if (tx >= p.ntx) return;
     uint16_t* nm = s_nm[warp];
     volatile uint16_t* vnm = nm;
-    volatile uint32_t* q = s_q[warp];
+    volatile uint16_t* q = s_q[warp];
     const int L = p.L, Lw = L >> 2;
     const int x0 = tx * TW, y0 = ty * TH;
-    const int tw_eff = FULLW ? TW : min(TW, L - x0), th_eff = FULLW ? TH : min(TH, L - y0);   // TH divides TW
+    const int tw_eff = FULLW ? TW : min(TW, L - x0), th_eff = min(TH, L - y0);
     const int x = x0 + 4 * lane;
     const bool colv = FULLW || 4 * lane < tw_eff;
     const int last_lane = (tw_eff >> 2) - 1;             // lane that owns the strip's last column
@@ -179,9 +328,10 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
     const int base = y0 * L + x0;
     const int xw = x >> 2;
     const int xew = ((x + 4 == L) ? 0 : x + 4) >> 2;     // east halo word of the last lane (periodic)
-    const unsigned lt = lanemask_lt(), me = 1u << lane, le = lt | me, gt = ~le;
+    const unsigned lt = lanemask_lt();
     // the east bond that leaves the strip is dropped from the lane's bond byte; lanes beyond a ragged edge have no bonds
     const uint32_t gmask = !colv ? 0u : is_last ? 0xBFu : 0xFFu;
+    const uint32_t left_ok = lane ? (F_LK | F_LC) : 0u;  // the first lane has no left neighbour
 
     // spin words of rows y, y+1, y+2 (w*) and the east halo words of the last lane (h*); row index L wraps to 0
     uint32_t w0 = 0, w1 = 0, w2 = 0, h0 = 0, h1 = 0, h2 = 0;
@@ -202,13 +352,13 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
     }
 
     uint32_t P01 = 0, P23 = 0;                           // names carried by the previous row's sites
-    uint32_t npm = 0;                                    // north bonds from the previous row into this row (bits 1,3,5,6)
+    uint32_t Gn = 0;                                     // north bonds of the previous row (bits 1,3,5,7 of its bond byte)
     uint32_t NEW01 = (uint32_t)(4 * lane) * 0x00010001u + 0x00010000u;      // own names of sites 0,1 / 2,3 of this row
     uint32_t NEW23 = NEW01 + 0x00020002u;
     uint32_t nact = 0;
-    int qn = 0;                                          // queued pairs (warp-uniform)
-    uint32_t eastm = 0;                                  // bit (th_eff-1-ly) = the east bond of site 3 in row ly (last lane: it leaves the strip)
-    uint32_t northm = 0;                                 // bond byte of the last row: its north bonds (bits 1,3,5,7) leave the strip
+    int qn = 0;                                          // queued entries (warp-uniform)
+    uint32_t fl = 0;                                     // mismatch flags, 4 per row, the newest row in bits 0..3
+    uint32_t fe = 0;                                     // link flags, 1 per row, the newest row in bit 0
 
     // running per-row quantities: Philox counter of the lane's first pair, global index of the lane's first site, pointer
     // to the lane's spin word of the row to prefetch (ly + 3)
@@ -217,11 +367,11 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
     const uint32_t* pw = spins_w + (size_t)(y0 + 3) * Lw + xws;   // the lane's word of the row to prefetch; halo: + dxe
     const uint32_t* const pw_halo = spins_w + row_halo + xws;
     const int dxe = xew - xws;
-
     uint32_t dw = 0;                                     // draw bytes of the rows 4g..4g+3 (SRC_DRAWS)
     const uint32_t* pdw = draws + (SRC == SRC_DRAWS ? draw_word_index(p, tx, ty, 0, lane) : 0);
+    uint32_t G = 0;                                      // the lane's bond byte of the current row
+
     for (int ly = 0; ly < th_eff; ++ly) {
-        uint32_t G = 0;                                  // the lane's bond byte of this row
         if (!FROM_BONDS) {
             uint32_t d;
             if (SRC == SRC_DRAWS && (ly & 3) == 0) { dw = *pdw; pdw += 32; }
@@ -240,43 +390,27 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
             G = bond_byte<ISING>(p, d, w0, east, w1);
             c0 += (uint32_t)L >> 1;
             w0 = w1; w1 = w2; w2 = w3; h0 = h1; h1 = h2; h2 = h3;
-        } else if (colv) {
-            G = bonds_in[(size_t)gi >> 2];
+        } else {
+            G = colv ? bonds_in[(size_t)gi >> 2] : 0u;
         }
-        // bonds that leave the strip are remembered for the edge arrays and dropped here
-        // (the north bonds of the last row are not used inside the loop: they only feed the next row's table index)
-        eastm = eastm * 2u + ((G >> 6) & 1u);
+        // the bond that leaves the strip to the east is remembered for the edge arrays and dropped here
+        if (is_last) s_e3[warp][ly] = (uint8_t)G;
         G &= gmask;
-        northm = G;
+        nact += __popc(G);
 
         // ---- names of this row's sites ----------------------------------------------------------------------
-        const uint32_t EL = (__shfl_up_sync(FULLM, G, 1) >> 5) & (lane ? 2u : 0u);
-        const uint4 A = s_la[(G & 0x15u) | npm];
-        const uint32_t Bf = s_lb[(G & 0x55u) | EL];
-        const uint32_t X = prmt(P01, P23, A.x);
-        uint32_t l01 = prmt(X, NEW01, A.x >> 16);
-        const uint32_t W = prmt(P23, NEW23, A.y);
-        uint32_t l23 = prmt(W, l01, A.y >> 16);
-        nact += A.w >> 28;
-
-        // runs that cross lane boundaries: lanes a..b, a's suffix segment, full lanes, b's prefix segment
-        const bool E3 = G & 0x40u;
-        const unsigned LINK = __ballot_sync(FULLM, E3);
-        const unsigned FULLB = __ballot_sync(FULLM, (G & 0x15u) == 0x15u);
-        const unsigned CS = __ballot_sync(FULLM, (A.w & 1u) != 0u);
-        const unsigned CP = __ballot_sync(FULLM, (A.w & 2u) != 0u);
-        const unsigned nPTL = ~(FULLB & (LINK << 1));                       // lanes where a run cannot pass to the left
-        const unsigned nPTR = ~(FULLB & LINK);                              // ... to the right
-        const int a_le = 31 - __clz(nPTL & le);                             // bit 0 of nPTL is always set
-        const int bS = E3 ? __ffs(nPTR & gt) - 1 : lane;                    // bit 31 of nPTR is always set
-        const unsigned MS = (CS & ((1u << bS) - 1u) & (FULLM << a_le)) | (CP & (1u << bS));
-        const int srcS = MS ? __ffs(MS) - 1 : a_le;                         // lane that holds the run's name
-        const uint32_t pub = prmt(l01, l23, 0x7610);                        // l0 | l3 << 16
-        const uint32_t v = __shfl_sync(FULLM, pub, srcS);
-        const uint32_t RS = prmt(v, 0u, srcS == bS ? 0x4410u : 0x4432u);    // the last lane's prefix name, else a suffix name
-        const uint32_t RPS = prmt(__shfl_up_sync(FULLM, RS, 1), RS, 0x5410);   // RP | RS << 16
-        l01 = prmt(l01, RPS, Bf);
-        l23 = prmt(l23, RPS, Bf >> 16);
+        const uint4 A4 = s_la[(G & 0x55u) | Gn];
+        const uint4 B4 = s_lb[G & 0x15u];
+        const uint32_t A[4] = {A4.x, A4.y, A4.z, A4.w}, B[4] = {B4.x, B4.y, B4.z, B4.w};
+        uint32_t l01, l23, to_right, to_left;
+        row_local(A, P01, P23, NEW01, NEW23, l01, l23, to_right, to_left);
+        const uint32_t from_left = __shfl_up_sync(FULLM, to_right, 1);
+        const uint32_t from_right = __shfl_down_sync(FULLM, to_left, 1);
+        const uint32_t link = row_final(A, B, from_left, from_right, left_ok, l01, l23);
+        // link flag -> fe = 2 fe + [link != 0]: (link + 0x30000) >> 18 on the multiply-add pipe
+        fe = mad_hi(link + 0x00030000u, 1u << 14, fe + fe);
+        // mismatch flags -> fl = 16 fl + flags
+        fl = mad_hi(row_mismatch(A, P01, P23, l01, l23), 1u << 16, mad_lo(fl, 16u, 0u));
 
         // the row's entries in the forest (a new node's name is its own index, i.e. it starts as a root) and in `prov`
         *reinterpret_cast<uint2*>(nm + ly * TW + 4 * lane) = make_uint2(l01, l23);
@@ -290,41 +424,22 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
             *reinterpret_cast<int4*>(prov + (size_t)gi) = g;
         }
 
-        // contacts whose carried name differs from the adopted one: queue the pair of names
-        {
-            const uint32_t d01 = (P01 ^ l01) & prmt(0x0000FFFFu, 0u, A.z);
-            const uint32_t d23 = (P23 ^ l23) & prmt(0x0000FFFFu, 0u, A.z >> 16);
-            const bool m0 = d01 & 0xFFFFu, m1 = d01 >> 16, m2 = d23 & 0xFFFFu, m3 = d23 >> 16;
-            const unsigned B0 = __ballot_sync(FULLM, m0), B1 = __ballot_sync(FULLM, m1);
-            const unsigned B2 = __ballot_sync(FULLM, m2), B3 = __ballot_sync(FULLM, m3);
-            volatile uint32_t* qp = q + qn;
-            if (m0) qp[__popc(B0 & lt)] = prmt(l01, P01, 0x5410);
-            qp += __popc(B0);
-            if (m1) qp[__popc(B1 & lt)] = prmt(l01, P01, 0x7632);
-            qp += __popc(B1);
-            if (m2) qp[__popc(B2 & lt)] = prmt(l23, P23, 0x5410);
-            qp += __popc(B2);
-            if (m3) qp[__popc(B3 & lt)] = prmt(l23, P23, 0x7632);
-            qp += __popc(B3);
-            qn = (int)(qp - q);
-        }
-        if (qn >= 32) {
-            __syncwarp();                                // queue, forest entries and `prov` rows visible to the whole warp
-            do {
-                qn -= 32;
-                unite_batch(vnm, true, q[qn + lane], prov, base, L);
-            } while (qn >= 32);
-            __syncwarp();                                // queue slots read before the next row overwrites them
+        if ((ly & 7) == 7) {                             // unite the names of the flagged sites of the last 8 rows
+            __syncwarp();
+            drain_flags(fl, 2, ly * TW + 4 * lane, 0u, q, qn, vnm, prov, base, L, lane, lt);
+            fl = 0;
         }
 
         P01 = l01; P23 = l23;
-        npm = (G & 0x2Au) | ((G >> 1) & 0x40u);
+        Gn = G & 0xAAu;
         NEW01 += (uint32_t)TW * 0x00010001u;
         NEW23 += (uint32_t)TW * 0x00010001u;
         gi += L;
     }
 
-    northm &= 0xAAu;
+    __syncwarp();
+    drain_flags(fl, 2, (th_eff - 1) * TW + 4 * lane, 0u, q, qn, vnm, prov, base, L, lane, lt);    // rows since the last drain
+    drain_flags(fe, 0, (th_eff - 1) * TW + 4 * lane, QEAST, q, qn, vnm, prov, base, L, lane, lt);  // link flags of all rows
     __syncwarp();
     if (qn > 0) {
         const bool have = lane < qn;
@@ -335,6 +450,7 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
     // ---- edge arrays: strip-local roots of the sites on the four edges ----------------------------------------------
     {
         const int nE = p.ntx * L;
+        const uint32_t northm = G;                       // bond byte of the last row: its north bonds leave the strip
         if (colv) {
             // first row -> rootS, last row -> rootN (-1 where the north bond that leaves the strip is not active)
             const int lb0 = 4 * lane, lb1 = (th_eff - 1) * TW + 4 * lane;
@@ -355,23 +471,21 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
             *reinterpret_cast<int4*>(edgeA + (size_t)nE + (size_t)ty * L + x) = n;
         }
         // first column -> rootW, last column -> rootE: lane i takes row i
-        const uint32_t em = __shfl_sync(FULLM, eastm, last_lane);           // row ly at bit th_eff-1-ly
+        uint32_t e3 = 0;
         if (lane < th_eff) {
+            e3 = s_e3[warp][lane] & 0x40u;
             int w = lane * TW, e = lane * TW + tw_eff - 1, w2 = w, e2 = e;
             nm_root4(vnm, w, e, w2, e2);
             edgeB[(size_t)tx * L + y0 + lane] = strip_gidx(base, L, w);
-            edgeA[(size_t)tx * L + y0 + lane] = ((em >> (th_eff - 1 - lane)) & 1u) ? strip_gidx(base, L, e) : -1;
+            edgeA[(size_t)tx * L + y0 + lane] = e3 ? strip_gidx(base, L, e) : -1;
         }
+        nact += e3 >> 6;                                 // the east bonds that leave the strip were masked before the count
     }
 
     if (!FROM_BONDS) {
-        nact += __popc(northm);
-        if (colv) nact += __popc(eastm);                 // my east bonds into the next lane / out of the strip, all rows
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) nact += __shfl_xor_sync(FULLM, nact, o);
+        nact = __reduce_add_sync(FULLM, nact);
         if (lane == 0 && nact)
             atomicAdd(&acc->part[(tx + 5 * ty) & (ACC_PARTS - 1)].n_active, (unsigned long long)nact);
     }
 }
-
 }  // namespace swb

@@ -1,6 +1,6 @@
-"""k_scan's permutation tables against the plain definition of run naming, on the host (-m "not gpu"): the table
-generator is constexpr C++ shared with the kernel (paper_1105_5804_b200/csrc/scan_kernel.cuh), the checker
-tests/host/scan_lut_check.cu emulates PRMT and enumerates every pattern."""
+"""k_scan's row logic against the plain definition of connectivity, on the host (-m "not gpu"): the naming tables
+(constexpr C++) and the per-lane row functions are shared with the kernel (paper_1105_5804_b200/csrc/scan_kernel.cuh);
+the checker tests/host/scan_row_check.cu emulates PRMT and the two shuffles and runs whole rows of lanes."""
 import os
 import subprocess
 import tempfile
@@ -8,12 +8,12 @@ import tempfile
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def test_scan_tables_match_the_definition_of_run_naming():
-    src = os.path.join(ROOT, "tests", "host", "scan_lut_check.cu")
+def test_scan_rows_match_the_definition_of_connectivity():
+    src = os.path.join(ROOT, "tests", "host", "scan_row_check.cu")
     with tempfile.TemporaryDirectory() as d:
-        exe = os.path.join(d, "scan_lut_check")
+        exe = os.path.join(d, "scan_row_check")
         cmd = ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O1", "-o", exe, src]
         r = subprocess.run(cmd, capture_output=True, text=True)
         assert r.returncode == 0, r.stderr
         r = subprocess.run([exe], capture_output=True, text=True)
-        assert r.returncode == 0 and "scan tables ok: 4096 cases" in r.stdout, r.stdout + r.stderr
+        assert r.returncode == 0 and "scan rows ok: 72000 rows" in r.stdout, r.stdout + r.stderr
