@@ -231,12 +231,21 @@ __device__ __forceinline__ size_t draw_word_index(const Params& p, int tx, int t
 // neighbour p - 1 (link flag), else of p and of the site above it, p - TW (mismatch flag).  Names are read back from the
 // forest array: entry of a site = the name it took (a node) or, for a node, its parent.
 constexpr uint32_t QEAST = 0x8000u;
-constexpr int QCAP = 64;                                 // < 32 entries carried over + at most 32 new ones per round
+#ifndef SWB_UNITE_V2
+#define SWB_UNITE_V2 1
+#endif
+#ifndef SWB_DRAIN_SCAN
+#define SWB_DRAIN_SCAN 1
+#endif
+// Queue capacity per warp: a drain appends all flagged sites of 8 rows at once when they fit (the usual case: about 100
+// at beta_c), else 32 at a time.
+constexpr int QCAP = SCAN_WARPS >= 8 ? 384 : 64;
 
 // Unite one queued pair per lane, hooking the larger root under the smaller and writing every hook through to `prov`.
-// 3-phase protocol, no atomics (the forest belongs to this warp): (1) all lanes find roots -- nobody hooks, so a root stays
-// a root; (2) hook with a plain store -- lanes hooking the same root collide, one store wins; (3) re-read: losers retry
-// from the new roots.
+// 3-phase protocol, no atomics (the forest belongs to this warp): (1) all lanes find the roots of their two names, the two
+// chases in lockstep, and point the two names directly at their roots (the same names keep coming back while a cluster
+// grows down the strip) -- nobody hooks, so a root stays a root; (2) hook with a plain store -- lanes hooking the same
+// root collide, one store wins; (3) re-read: losers retry from the new roots.
 __device__ __forceinline__ void unite_batch(volatile uint16_t* nm, bool have, uint32_t code, int* prov, int base, int L)
 {
     int ua = 0, ub = 0;
@@ -247,8 +256,19 @@ __device__ __forceinline__ void unite_batch(volatile uint16_t* nm, bool have, ui
     }
     while (__any_sync(FULLM, have)) {
         if (have) {
+#if SWB_UNITE_V2
+            const int a0 = ua, b0 = ub;
+            int pa = nm[ua], pb = nm[ub];
+            while ((pa ^ ua) | (pb ^ ub)) {
+                ua = pa; ub = pb;
+                pa = nm[ua]; pb = nm[ub];
+            }
+            if (a0 != ua) nm[a0] = (uint16_t)ua;
+            if (b0 != ub) nm[b0] = (uint16_t)ub;
+#else
             ua = nm_find(nm, ua);
             ub = nm_find(nm, ub);
+#endif
             if (ua == ub) have = false;
             else if (ua < ub) { const int t = ua; ua = ub; ub = t; }
         }
@@ -262,12 +282,39 @@ __device__ __forceinline__ void unite_batch(volatile uint16_t* nm, bool have, ui
     }
 }
 
-// Collect the flagged sites of a lane's flag word into the warp's queue and unite them 32 at a time.  Bit b of `flags`
+// Collect the flagged sites of the lanes' flag words into the warp's queue and unite them 32 at a time.  Bit b of `flags`
 // stands for the strip-local position pos0 - (b >> sh) * TW + (b & ((1 << sh) - 1)) (sh = 2: 4 mismatch flags per row, the
-// newest row in bits 0..3; sh = 0: one link flag per row) | tag.  Every round each lane that still has a flag appends one.
+// newest row in bits 0..3; sh = 0: one link flag per row) | tag.  If all of them fit into the queue, a warp scan of the
+// per-lane counts gives every lane its slots and it appends its own entries; else every round each lane that still has a
+// flag appends one and full batches are united on the way.
 __device__ __forceinline__ void drain_flags(uint32_t flags, int sh, int pos0, uint32_t tag, volatile uint16_t* q, int& qn,
                                             volatile uint16_t* nm, int* prov, int base, int L, int lane, unsigned lt)
 {
+    const int cnt = __popc(flags);
+    int incl = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(FULLM, incl, o);
+        if (lane >= o) incl += t;
+    }
+    const int total = __shfl_sync(FULLM, incl, 31);
+    if (total == 0) return;
+    if (SWB_DRAIN_SCAN && total <= QCAP - qn) {
+        volatile uint16_t* out = q + qn + (incl - cnt);
+        while (flags) {
+            const int b = 31 - __clz(flags);
+            flags ^= 1u << b;
+            *out++ = (uint16_t)((uint32_t)(pos0 - ((b >> sh) << TW_LOG) + (b & ((1 << sh) - 1))) | tag);
+        }
+        qn += total;
+        __syncwarp();                                    // queue entries and forest rows visible to the whole warp
+        while (qn >= 32) {
+            qn -= 32;
+            unite_batch(nm, true, q[qn + lane], prov, base, L);
+        }
+        __syncwarp();                                    // queue slots read before they are overwritten
+        return;
+    }
     while (true) {
         const bool has = flags != 0u;
         const unsigned Bm = __ballot_sync(FULLM, has);
@@ -279,33 +326,48 @@ __device__ __forceinline__ void drain_flags(uint32_t flags, int sh, int pos0, ui
             q[qn + __popc(Bm & lt)] = (uint16_t)((uint32_t)pos | tag);
         }
         qn += __popc(Bm);
-        if (qn >= 32) {
-            __syncwarp();                                // queue entries and forest rows visible to the whole warp
+        __syncwarp();
+        while (qn >= 32) {
             qn -= 32;
             unite_batch(nm, true, q[qn + lane], prov, base, L);
-            __syncwarp();                                // queue slots read before they are overwritten
         }
+        __syncwarp();
     }
 }
 
 // ---------------------------------------------------------------------------------------------------- k_scan
+#ifndef SWB_SCAN_UNROLL
+#define SWB_SCAN_UNROLL 2
+#endif
+constexpr int SCAN_UNROLL = SWB_SCAN_UNROLL;
+
+struct ScanSmem {
+    uint16_t nm[SCAN_WARPS][TW * TH];                    // the strips' forests
+    uint4    la[256];                                    // naming tables
+    uint4    lb[22];
+    uint16_t q[SCAN_WARPS][QCAP];                        // queues of flagged sites
+    uint8_t  e3[SCAN_WARPS][TH];                         // bond byte of the strip's last lane, row by row (bit 6 leaves the strip)
+#ifdef SWB_SCAN_PAD
+    uint8_t  pad[SWB_SCAN_PAD];
+#endif
+};
+
 // SRC_PHILOX: read spins, draw bonds (a1).  SRC_DRAWS: read spins and the draw cache k_final filled one sweep ahead (the
 // same bonds, the Philox work done elsewhere).  SRC_BONDS: read packed bonds (sw_label).  Writes the provisional labels
 // (`prov`, see label_kernels.cuh) and the edge arrays, and adds the number of active bonds to the sweep counters.
 // FULLW: L is a multiple of TW, every strip has all 32 lanes (no ragged right edge; the predicates fold away).
 enum { SRC_PHILOX = 0, SRC_BONDS = 1, SRC_DRAWS = 2 };
 template <int SRC, bool ISING, bool FULLW>
-__global__ void __launch_bounds__(SCAN_THREADS)
+__global__ void __launch_bounds__(SCAN_THREADS, 24 / SCAN_WARPS)    // 24 warps per SM (shared memory): up to 85 registers
 k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __restrict__ bonds_in,
        const uint32_t* __restrict__ draws, int* prov, int* __restrict__ edgeA, int* __restrict__ edgeB,
        Acc* __restrict__ acc)
 {
     constexpr bool FROM_BONDS = SRC == SRC_BONDS;
-    __shared__ __align__(16) uint16_t s_nm[SCAN_WARPS][TW * TH];
-    __shared__ __align__(16) uint4 s_la[256];
-    __shared__ __align__(16) uint4 s_lb[22];
-    __shared__ uint16_t s_q[SCAN_WARPS][QCAP];
-    __shared__ uint8_t s_e3[SCAN_WARPS][TH];             // bond byte of the strip's last lane, row by row (bit 6 leaves the strip)
+    extern __shared__ __align__(16) unsigned char s_raw[];   // ScanSmem: more than the 48 KB a static allocation may have
+    ScanSmem& sm = *reinterpret_cast<ScanSmem*>(s_raw);
+    uint4* const s_la = sm.la;
+    uint4* const s_lb = sm.lb;
     for (int i = threadIdx.x; i < 256; i += SCAN_THREADS)
         s_la[i] = make_uint4(d_scan_lut.a[i][0], d_scan_lut.a[i][1], d_scan_lut.a[i][2], d_scan_lut.a[i][3]);
     for (int i = threadIdx.x; i < 22; i += SCAN_THREADS)
@@ -315,9 +377,10 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int tx = blockIdx.x * SCAN_WARPS + warp, ty = blockIdx.y;
     if (tx >= p.ntx) return;
-    uint16_t* nm = s_nm[warp];
+    uint16_t* nm = sm.nm[warp];
     volatile uint16_t* vnm = nm;
-    volatile uint16_t* q = s_q[warp];
+    volatile uint16_t* q = sm.q[warp];
+    uint8_t* const s_e3 = sm.e3[warp];
     const int L = p.L, Lw = L >> 2;
     const int x0 = tx * TW, y0 = ty * TH;
     const int tw_eff = FULLW ? TW : min(TW, L - x0), th_eff = min(TH, L - y0);
@@ -371,6 +434,9 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
     const uint32_t* pdw = draws + (SRC == SRC_DRAWS ? draw_word_index(p, tx, ty, 0, lane) : 0);
     uint32_t G = 0;                                      // the lane's bond byte of the current row
 
+    // (Computing the bond byte, or only its Philox draws, one row ahead of the naming chain -- software pipelining inside
+    // the warp -- was measured slower: 0.88 -> 0.91 / 1.01 ms; the other warps of the sub-partition hide that latency.)
+#pragma unroll SCAN_UNROLL
     for (int ly = 0; ly < th_eff; ++ly) {
         if (!FROM_BONDS) {
             uint32_t d;
@@ -394,7 +460,7 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
             G = colv ? bonds_in[(size_t)gi >> 2] : 0u;
         }
         // the bond that leaves the strip to the east is remembered for the edge arrays and dropped here
-        if (is_last) s_e3[warp][ly] = (uint8_t)G;
+        if (is_last) s_e3[ly] = (uint8_t)G;
         G &= gmask;
         nact += __popc(G);
 
@@ -473,7 +539,7 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
         // first column -> rootW, last column -> rootE: lane i takes row i
         uint32_t e3 = 0;
         if (lane < th_eff) {
-            e3 = s_e3[warp][lane] & 0x40u;
+            e3 = s_e3[lane] & 0x40u;
             int w = lane * TW, e = lane * TW + tw_eff - 1, w2 = w, e2 = e;
             nm_root4(vnm, w, e, w2, e2);
             edgeB[(size_t)tx * L + y0 + lane] = strip_gidx(base, L, w);

@@ -147,7 +147,16 @@ int launch_label_front(sw_handle* h, const Params& p, const uint8_t* bonds, int3
                                 : (fullw ? k_scan<SRC_DRAWS, false, true> : k_scan<SRC_DRAWS, false, false>))
                        : (ising ? (fullw ? k_scan<SRC_PHILOX, true, true> : k_scan<SRC_PHILOX, true, false>)
                                 : (fullw ? k_scan<SRC_PHILOX, false, true> : k_scan<SRC_PHILOX, false, false>));
-    kern<<<grid, SCAN_THREADS, 0, s>>>(p, h->d_spins, bonds, h->d_draws, labels, h->d_edgeA, h->d_edgeB, h->d_acc);
+    static const void* opted[16];                        // kernels whose dynamic shared-memory limit has been raised
+    static int nopted = 0;
+    bool done = false;
+    for (int i = 0; i < nopted; ++i) done = done || opted[i] == (const void*)kern;
+    if (!done) {
+        SW_CUDA(h, cudaFuncSetAttribute((const void*)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(ScanSmem)));
+        if (nopted < 16) opted[nopted++] = (const void*)kern;
+    }
+    kern<<<grid, SCAN_THREADS, sizeof(ScanSmem), s>>>(p, h->d_spins, bonds, h->d_draws, labels, h->d_edgeA, h->d_edgeB,
+                                                      h->d_acc);
     SW_LAUNCHED(h, "k_scan");
     SW_PROF(h, 1, s);
     const int nseam = (p.ntx + p.nty) * p.L;
