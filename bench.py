@@ -28,13 +28,39 @@ PAPER_NS_L16384 = 3.573          # Table I, Tesla M2070, q=2,
 BYTES_PER_SITE_SWEEP = 14.0      # SURVEY 8(d) model (iii) / DESIGN.md: 1 + 4 + 4 + 4 + 1
 BYTES_PER_SITE = {"k_scan": 5.0, "k_seam": 0.0, "k_final": 9.0}   # DESIGN.md per-kernel table
 PHASES = ["k_scan", "k_seam", "k_final"]
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture
-# (profiles/r01c_README.md), bytes, at L=16384 beta_c; None for other sizes.
-NCU_TRAFFIC = {"k_scan": 0.268577e9 + 1.101891e9, "k_seam": 0.328467e9 + 0.053556e9, "k_final": 1.073818e9 + 1.282418e9}
-# smsp__inst_executed.sum per launch from the same capture: the kernels are instruction-issue bound
-NCU_WARP_INST = {"k_scan": 784.67e6, "k_seam": 38.71e6, "k_final": 421.62e6}
+# ncu counters per launch (dram bytes, warp instructions) are NOT constants of this file: they are read from the tracked
+# capture profiles/r02_counters.json, which records the hash of the kernel sources it was taken on; if the sources have
+# changed since, the fields are reported as null with the reason (ncu_counters below).
+COUNTERS_FILE = os.path.join(ROOT, "profiles", "r02_counters.json")
+EQUIL_SWEEPS = 100               # untimed sweeps before the timed region: SURVEY 8(d) "time sweeps 50-200", equilibrium state
 N_SMSP = 148 * 4
 BYTES_PER_SITE_LABEL = 12.25     # sw_label alone = packed bonds 0.25 + 4 + 4 + 4
+
+
+def kernel_source_hash() -> str:
+    """sha256 over the CUDA sources of the library (the GPU box has no .git: a content hash stands in for the commit)."""
+    import glob
+    import hashlib
+    h = hashlib.sha256()
+    for f in sorted(glob.glob(os.path.join(ROOT, "paper_1105_5804_b200", "csrc", "*"))):
+        with open(f, "rb") as fh:
+            h.update(os.path.basename(f).encode() + b"\0" + fh.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_counters(L: int, beta: float):
+    """-> (counters per kernel or None, source string)"""
+    try:
+        with open(COUNTERS_FILE) as f:
+            c = json.load(f)
+    except Exception:
+        return None, "none: profiles/r02_counters.json absent"
+    if c.get("source_sha") != kernel_source_hash():
+        return None, "stale: profiles/r02_counters.json was captured on kernel sources %s, this run has %s" % (
+            c.get("source_sha"), kernel_source_hash())
+    if c.get("L") != L or abs(c.get("beta", -1.0) - beta) > 1e-6:
+        return None, "profiles/r02_counters.json is for L=%s beta=%s" % (c.get("L"), c.get("beta"))
+    return c["kernels"], "profiles/r02_counters.json (ncu --set full, %s, kernel sources %s)" % (c.get("captured"), c.get("source_sha"))
 
 
 def beta_c_ising() -> float:
@@ -187,8 +213,18 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    def state_of(l):
+        o = l.observables()
+        return {"energy_per_site": o["energy"] / N, "magnetisation_per_site": o["magnetisation"] / N,
+                "clusters_per_site": o["n_clusters"] / N, "largest_cluster_fraction": o["max_cluster"] / N,
+                "counter": o["counter"]}
+
     # ---- device-resident timing ----------------------------------------------------------------------------
+    # the timed configurations are equilibrium ones whatever --warmup says: at least EQUIL_SWEEPS
+    # untimed sweeps from the random start, then the W warm-up sweeps of the contract, then the K timed ones
+    lat.sweep(max(0, EQUIL_SWEEPS - args.warmup))
     lat.sweep(args.warmup)
+    state_before = state_of(lat) if rank == 0 else None
     barrier()
     sampler = ClockSampler(local_rank)
     if rank == 0:
@@ -214,7 +250,7 @@ def run_ours(args):
     phase_ms, nprof = lat.profile_read()
     lat.profile_enable(False)
     per_kernel = {name: phase_ms[i] / max(1, nprof) for i, name in enumerate(PHASES)}
-    obs = lat.observables()
+    state_after = state_of(lat) if rank == 0 else None
 
     # ---- labelling alone (BASELINE.json configs[3], metric "labelling GB/s"): bond percolation at p = 1/2 --------------
     labelling = None
@@ -259,21 +295,23 @@ def run_ours(args):
 
     # ---- the other temperatures of BASELINE.json configs[2] (short runs; the headline stays beta_c) -------------------
     other_betas = None
-    if rank == 0 and args.all_betas:
+    if rank == 0 and not args.no_other_betas:
         other_betas = {}
         for b in (0.40, 0.50):
             lb = binding.Lattice(L, 2, b, 1, device=device)
             lb.init_spins(1)
-            lb.sweep(60)
+            lb.sweep(EQUIL_SWEEPS)
             torch.cuda.synchronize()
             ev0.record(stream)
-            lb.sweep(40)
+            lb.sweep(100)
             ev1.record(stream)
             torch.cuda.synchronize()
-            ms = ev0.elapsed_time(ev1) / 40
-            lb.profile_enable(True); lb.sweep(20); ph, nb = lb.profile_read(); lb.profile_enable(False)
+            ms = ev0.elapsed_time(ev1) / 100
+            lb.profile_enable(True); lb.sweep(50); ph, nb = lb.profile_read(); lb.profile_enable(False)
             other_betas["%.2f" % b] = {"ms_per_step": ms, "ns_per_spin_update": ms * 1e6 / N,
-                                       "kernel_ms": {name: ph[i] / max(1, nb) for i, name in enumerate(PHASES)}}
+                                       "frac_of_8TBps_nominal": BYTES_PER_SITE_SWEEP * N / (ms * 1e-3) / 1e9 / 8000.0,
+                                       "kernel_ms": {name: ph[i] / max(1, nb) for i, name in enumerate(PHASES)},
+                                       "state": state_of(lb)}
             lb.close()
 
     # ---- end to end through the host-buffer entry point ----------------------------------------------------
@@ -303,8 +341,10 @@ def run_ours(args):
     dom = max(("k_scan", "k_final"), key=lambda k: per_kernel[k])
     dom_bytes = BYTES_PER_SITE[dom] * N
     achieved = dom_bytes / (per_kernel[dom] * 1e-3) / 1e9
+    counters, counters_src = ncu_counters(L, beta)
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": NCU_TRAFFIC.get(dom) if L == 16384 else None, "peak_source": peak_src,
+                "frac": achieved / peak, "traffic": counters[dom]["dram_bytes"] if counters else None,
+                "traffic_source": counters_src, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": dom_bytes, "kernel_ms": per_kernel[dom],
                 "kernel_ms_all": per_kernel,
                 "kernel_share_of_step": per_kernel[dom] / max(1e-12, sum(per_kernel.values())),
@@ -314,32 +354,39 @@ def run_ours(args):
                           "frac_of_8TBps_nominal": BYTES_PER_SITE_SWEEP * N / (ms_per_step * 1e-3) / 1e9 / 8000.0,
                           "frac_compulsory_6B_of_measured_peak": 6.0 * N / (ms_per_step * 1e-3) / 1e9 / peak}}
 
-    if L == 16384 and clocks and clocks.get("sm_mhz"):
+    if counters and clocks and clocks.get("sm_mhz"):
         # issue-slot view: warp instructions per launch (ncu) / (SM sub-partitions x clock x kernel time); peak 1 per cycle
-        roofline["alu"] = {name: {"warp_inst": NCU_WARP_INST[name],
-                                  "issue_frac": NCU_WARP_INST[name] / (N_SMSP * clocks["sm_mhz"] * 1e6 * per_kernel[name] * 1e-3)}
+        roofline["alu"] = {name: {"warp_inst": counters[name]["warp_inst"],
+                                  "issue_frac": counters[name]["warp_inst"] / (N_SMSP * clocks["sm_mhz"] * 1e6 * per_kernel[name] * 1e-3)}
                            for name in PHASES}
 
     # ---- the oracle on this box's host cores, bounded sample ---------------------------------------------------
     cpu = None
     if not args.no_cpu_baseline:
-        Ls = min(L, 4096)
-        lat_s = binding.Lattice(Ls, 2, beta, 1, device=device)
-        lat_s.init_spins(1)
-        lat_s.sweep(60)                                               # equilibrate the sample on the GPU
-        s = lat_s.spins_host().copy()
-        lat_s.close()
+        # the oracle as it stands, one thread, on the workload itself -- 3 sweeps of the L x L lattice from the
+        # equilibrated GPU state (about 15 s each at L=16384).  Smaller budgets (--cpu-sweeps 0) fall back to an L=4096 sample.
         import oracle
         T = oracle.threshold(2, beta)
-        nsw = 12 if Ls >= 4096 else 24
+        if args.cpu_sweeps > 0:
+            Ls, nsw = L, args.cpu_sweeps
+            s = lat.spins_host().copy()
+            t_start = lat.get_counter()
+        else:
+            Ls, nsw = min(L, 4096), 12
+            lat_s = binding.Lattice(Ls, 2, beta, 1, device=device)
+            lat_s.init_spins(1)
+            lat_s.sweep(EQUIL_SWEEPS)
+            s = lat_s.spins_host().copy()
+            t_start = lat_s.get_counter()
+            lat_s.close()
         t0 = time.perf_counter()
         for k in range(nsw):
-            oracle.sweep(Ls, 2, T, 1, 60 + k, s)
+            oracle.sweep(Ls, 2, T, 1, t_start + k, s)
         dt = time.perf_counter() - t0
         cpu = {"value": dt / nsw / (Ls * Ls) * 1e9, "unit": "ns", "cores": 1, "kind": "oracle",
-               "sample": "%d serial oracle sweeps of an L=%d lattice at the same beta, started from a state "
-                         "equilibrated by 60 GPU sweeps (%.1f s of CPU work; host has %d cores, the oracle uses 1)"
-                         % (nsw, Ls, dt, os.cpu_count() or 0)}
+               "sample": "%d serial oracle sweeps of the L=%d lattice at the same beta, started from the state the GPU "
+                         "chain had reached after %d sweeps (%.1f s of CPU work; host has %d cores, the oracle uses 1; "
+                         "built %s)" % (nsw, Ls, t_start, dt, os.cpu_count() or 0, oracle.build_flags())}
 
     line = {
         "metric": "ns_per_spin_update", "value": ns_per_spin, "unit": "ns", "n_gpus": world, "steps": args.steps,
@@ -351,6 +398,7 @@ def run_ours(args):
                    "L": L, "q": 2, "beta": beta, "sites_per_step": N, "replicas": world,
                    "l2_policy": "inputs larger than L2: spins %d MiB + labels %d MiB per step vs 126 MB L2"
                                 % (N >> 20, (4 * N) >> 20),
+                   "equilibration": "%d untimed sweeps from the random start before the timed region" % max(EQUIL_SWEEPS, args.warmup),
                    "sweeps_per_s": 1e3 / ms_per_step * world},
         "clocks": clocks,
         "e2e": {"value": e2e_ns, "unit": "ns", "h2d_bytes_per_step": N, "d2h_bytes_per_step": N + 128,
@@ -361,9 +409,8 @@ def run_ours(args):
         "cpu_baseline": cpu,
         "labelling": labelling,
         "other_betas": other_betas,
-        "state": {"energy_per_site": obs["energy"] / N, "magnetisation_per_site": obs["magnetisation"] / N,
-                  "clusters_per_site": obs["n_clusters"] / N, "largest_cluster_fraction": obs["max_cluster"] / N,
-                  "counter": obs["counter"]},
+        "state_before_timed_region": state_before,
+        "state": state_after,
     }
     print(json.dumps(line), flush=True)
     lat.close()
@@ -383,7 +430,8 @@ def main(argv=None):
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-labelling", action="store_true")
-    ap.add_argument("--all-betas", action="store_true")
+    ap.add_argument("--no-other-betas", action="store_true", help="skip the beta = 0.40 / 0.50 legs of BASELINE.json configs[2]")
+    ap.add_argument("--cpu-sweeps", type=int, default=3, help="oracle sweeps of the full lattice for cpu_baseline (0: L=4096 sample)")
     args = ap.parse_args(argv)
     if args.warmup < 3:
         args.warmup = 3

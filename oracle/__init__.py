@@ -21,15 +21,35 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "sw_oracle.c")
-_LIB = os.path.join(_HERE, "libsw_oracle.so")
+
+
+def _machine_tag() -> str:
+    """The library is built -O3 -march=native (SURVEY.md 8(d) "CPU baseline beside it"), so it is tied to the CPU it was
+    built on: one file per CPU model, rebuilt where it is missing (the GPU box has gcc; the in-tree .so travels with the
+    repository snapshot but may come from another CPU)."""
+    import hashlib
+    try:
+        with open("/proc/cpuinfo") as f:
+            txt = "".join(l for l in f if l.startswith(("model name", "flags")))[:20000]
+    except OSError:
+        txt = "unknown"
+    return hashlib.sha256(txt.encode()).hexdigest()[:10]
+
+
+_FLAGS = ["-O3", "-march=native"]
+_LIB = os.path.join(_HERE, "libsw_oracle.%s.so" % _machine_tag())
+
+
+def build_flags() -> str:
+    return "gcc " + " ".join(_FLAGS)
 
 
 def build(force: bool = False) -> str:
-    """Compile sw_oracle.c with gcc (generic x86-64, so the .so also runs on the GPU box)."""
+    """Compile sw_oracle.c with gcc -O3 -march=native for this machine (integer code: the flags change no result)."""
     if force or (not os.path.exists(_LIB)) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         tmp = _LIB + ".tmp.%d" % os.getpid()
-        subprocess.check_call(["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-Wall", "-Wextra",
-                               "-o", tmp, _SRC, "-lm"])
+        subprocess.check_call(["gcc"] + _FLAGS + ["-std=c11", "-fPIC", "-shared", "-Wall", "-Wextra",
+                                                  "-o", tmp, _SRC, "-lm"])
         os.replace(tmp, _LIB)
     return _LIB
 
