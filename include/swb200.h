@@ -141,6 +141,17 @@ int sw_observables(sw_handle* h, sw_obs* h_out, void* stream);
 enum { SW_OBS_SPINS = 1, SW_OBS_CLUSTERS = 2 };
 int sw_observables_ex(sw_handle* h, sw_obs* h_out, int flags, void* stream);
 
+/* Energy and magnetisation of every configuration a chain passes through, at no extra pass over the spins (S:8a a6;
+ * BASELINE.json north_star (5) "a fused energy/magnetisation reduction"): the sweep's scan kernel reads every spin and
+ * its two neighbours anyway, so it counts the satisfied bonds and the minus spins of the configuration the sweep (or
+ * Wolff step) STARTS from.  The totals of the last 4096 consecutive sweeps / steps are kept on the device, filed under
+ * the step counter t the configuration belongs to (t = the number of sweeps / steps performed before it).
+ * sw_series_read copies n of them, counters t_first .. t_first + n - 1, to the host: energy as in sw_obs; magnetisation
+ * = sum_i s_i for q = 2 (h_magnetisation must be NULL for q > 2: state counts are not recorded on the sweep path).
+ * SW_EINVAL if a requested counter is not (or no longer) recorded: only counters of sweeps already performed are --
+ * the CURRENT configuration has not been scanned yet (use sw_observables_ex for it).  Synchronises `stream`. */
+int sw_series_read(sw_handle* h, uint64_t t_first, int64_t n, int64_t* h_energy, int64_t* h_magnetisation, void* stream);
+
 /* Host-buffer convenience for end-to-end use: copy h_spins_in (N bytes, may be NULL to keep the device state)
  * to the device, run n sweeps, copy spins back to h_spins_out (may be NULL) and labels to h_labels_out (may be
  * NULL), fill h_obs (may be NULL).  Synchronises `stream`. */

@@ -20,7 +20,7 @@ NPHASE = 3                                                # SW_NPHASE of include
 SYMBOLS = [
     "sw_create", "sw_destroy", "sw_workspace_bytes", "sw_bind", "sw_set_threshold", "sw_get_threshold",
     "sw_set_counter", "sw_get_counter", "sw_init_spins", "sw_sweep", "sw_activate", "sw_label",
-    "sw_cluster_stats", "wolff_step", "sw_observables", "sw_observables_ex", "sw_sweep_host", "sw_launch_count", "sw_strerror",
+    "sw_cluster_stats", "wolff_step", "sw_observables", "sw_observables_ex", "sw_series_read", "sw_sweep_host", "sw_launch_count", "sw_strerror",
     "sw_last_cuda_error", "sw_profile_enable", "sw_profile_read",
 ]
 
@@ -76,6 +76,7 @@ def lib():
     L.wolff_step.argtypes = [vp, i64, C.POINTER(i64), vp]
     L.sw_observables.argtypes = [vp, C.POINTER(sw_obs), vp]
     L.sw_observables_ex.argtypes = [vp, C.POINTER(sw_obs), C.c_int, vp]
+    L.sw_series_read.argtypes = [vp, u64, i64, C.POINTER(i64), C.POINTER(i64), vp]
     L.sw_sweep_host.argtypes = [vp, vp, i64, vp, vp, C.POINTER(sw_obs), vp]
     L.sw_launch_count.argtypes = [vp, C.POINTER(u64)]
     L.sw_profile_enable.argtypes = [vp, C.c_int]
@@ -194,6 +195,13 @@ class Lattice:
             flags = (OBS_SPINS if spins else 0) | (OBS_CLUSTERS if clusters else 0)
             self._check(self._lib.sw_observables_ex(self._h, C.byref(out), flags, self._stream()))
         return out.as_dict()
+
+    def series(self, t_first: int, n: int, magnetisation: bool = True):
+        """-> (energies, magnetisations or None) of the configurations at counters t_first .. t_first + n - 1"""
+        E = (C.c_int64 * n)()
+        M = (C.c_int64 * n)() if magnetisation else None
+        self._check(self._lib.sw_series_read(self._h, t_first, n, E, M, self._stream()))
+        return list(E), (list(M) if magnetisation else None)
 
     def sweep_host(self, h_spins_in, n: int, h_spins_out=None, h_labels_out=None, want_obs: bool = True):
         """Host-buffer end-to-end call: torch CPU tensors (ideally pinned) in and out."""

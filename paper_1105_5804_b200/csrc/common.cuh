@@ -102,7 +102,9 @@ constexpr int ACC_PARTS = 32;
 struct AccPart {                       // one 128-byte line per part: same-address atomics serialise in one L2 slice
     unsigned long long n_active;       // bonds activated by the last sweep / step
     unsigned long long n_clusters;     // roots counted by the last flatten pass
-    unsigned long long pad[14];
+    unsigned long long sat;            // satisfied bonds / sites in state 1 of the configuration the last sweep STARTED from
+    unsigned long long minus;          // (counted by k_scan from the spins it reads anyway; q = 2 only for `minus`)
+    unsigned long long pad[12];
 };
 struct Acc {
     AccPart part[ACC_PARTS];           // per-sweep counters: the sum over the parts is the value
@@ -114,5 +116,7 @@ struct Acc {
     unsigned long long hist[32];
 };
 constexpr int WOLFF_RING = 1024;       // per-step |C| slots between host flushes
+constexpr int SERIES_RING = 4096;      // sweeps whose (sat, minus) are kept for sw_series_read
+struct SeriesEntry { unsigned long long sat, minus; };
 
 }  // namespace swb

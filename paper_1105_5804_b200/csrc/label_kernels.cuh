@@ -172,9 +172,18 @@ __host__ __device__ inline int seam_part(int nseam)     // ids per part, a multi
     return ((nseam + 32 * SEAM_PER_THREAD - 1) / (32 * SEAM_PER_THREAD)) * 32;
 }
 
+// series != NULL (a sweep): one thread also files the (sat, minus) totals k_scan has just accumulated under the sweep's
+// counter, so that a chain keeps the energy and magnetisation of every configuration it passes through (sw_series_read).
 __global__ void __launch_bounds__(256)
-k_seam(const Params p, const int* __restrict__ edgeA, const int* __restrict__ edgeB, int* prov)
+k_seam(const Params p, const int* __restrict__ edgeA, const int* __restrict__ edgeB, int* prov,
+       const Acc* __restrict__ acc, SeriesEntry* __restrict__ series)
 {
+    if (series != nullptr && blockIdx.x == 0 && threadIdx.x == 0) {
+        unsigned long long sat = 0, minus = 0;
+        for (int k = 0; k < ACC_PARTS; ++k) { sat += acc->part[k].sat; minus += acc->part[k].minus; }
+        SeriesEntry e; e.sat = sat; e.minus = minus;
+        series[p.t_lo & (SERIES_RING - 1)] = e;
+    }
     const int nE = p.ntx * p.L, nseam = (p.ntx + p.nty) * p.L;
     const int part = seam_part(nseam);
     const int id = blockIdx.x * blockDim.x + threadIdx.x;

@@ -46,7 +46,8 @@ k_activate(const Params p, const uint32_t* __restrict__ spins_w, uint8_t* __rest
             const uint32_t wn = spins_w[(yy + 1 == L ? 0 : yy + 1) * Lw + xw];
             // (i>>1) of the first pair of this word = 2 * i4
             const uint32_t d = draw_byte(p, (uint32_t)i4 * 2u, p.t_lo, p.t_hi);
-            out |= bond_byte<ISING>(p, d, w, __funnelshift_r(w, we, 8), wn) << (8 * k);
+            uint32_t ce, cn;
+            out |= bond_byte<ISING>(p, d, w, __funnelshift_r(w, we, 8), wn, ce, cn) << (8 * k);
         }
         reinterpret_cast<uint32_t*>(bonds)[i16] = out;
     }

@@ -204,18 +204,32 @@ __device__ __forceinline__ uint32_t draw_byte(const Params& p, uint32_t c0, uint
 // format of include/swb200.h), for the 4 sites whose spins are w; e = spins of the east neighbours, n = of the north;
 // d = their draw byte.
 template <bool ISING>
-__device__ __forceinline__ uint32_t bond_byte(const Params& p, uint32_t d, uint32_t w, uint32_t e, uint32_t n)
+__device__ __forceinline__ uint32_t bond_byte(const Params& p, uint32_t d, uint32_t w, uint32_t e, uint32_t n,
+                                              uint32_t& ce, uint32_t& cn)
 {
+    // ce / cn: one bit per site (bit 8j+1 / 8j+2) that tells whether the east / north bond of site j is UNsatisfied (Ising)
+    // or satisfied (Potts); the caller adds them up byte-wise over the rows of a strip (the fused energy count)
     uint32_t eq;                                         // bit 8j+1: s_j == s_east, bit 8j+2: s_j == s_north
     if (ISING) {                                         // bytes 0x01 / 0xFF: equal <=> bit 1 (and bit 2) of the xor is 0
-        eq = (~(w ^ e) & 0x02020202u) | (~(w ^ n) & 0x04040404u);
+        ce = (w ^ e) & 0x02020202u;
+        cn = (w ^ n) & 0x04040404u;
+        eq = ~(ce | cn) & 0x06060606u;
     } else {
-        eq = (__vcmpeq4(w, e) & 0x02020202u) | (__vcmpeq4(w, n) & 0x04040404u);
+        ce = __vcmpeq4(w, e) & 0x02020202u;
+        cn = __vcmpeq4(w, n) & 0x04040404u;
+        eq = ce | cn;
     }
     // gather the 4 bit pairs (8j+1, 8j+2) into bits (2j, 2j+1) of the high word; the cross terms of the product land on
     // distinct bits below 32 or above bit 7 of the high word (no carries)
     // p.dmask = 0xFF, or 0 if T = 0 (then u >= T always, but u + 2^32 never carries)
     return __umulhi(eq, 0x82082000u) & ~d & p.dmask;     // 2^31 + 2^25 + 2^19 + 2^13
+}
+
+// sum of the 4 bytes of x
+__device__ __forceinline__ uint32_t byte_sum(uint32_t x)
+{
+    x = (x & 0x00FF00FFu) + ((x >> 8) & 0x00FF00FFu);
+    return (x + (x >> 16)) & 0xFFFFu;
 }
 
 // Draw cache (workspace): one 32-bit word per lane and group of 4 rows of a strip, byte r = draw byte of row 4g + r:
@@ -337,7 +351,7 @@ __device__ __forceinline__ void drain_flags(uint32_t flags, int sh, int pos0, ui
 
 // ---------------------------------------------------------------------------------------------------- k_scan
 #ifndef SWB_SCAN_UNROLL
-#define SWB_SCAN_UNROLL 2
+#define SWB_SCAN_UNROLL 1
 #endif
 constexpr int SCAN_UNROLL = SWB_SCAN_UNROLL;
 
@@ -419,6 +433,7 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
     uint32_t NEW01 = (uint32_t)(4 * lane) * 0x00010001u + 0x00010000u;      // own names of sites 0,1 / 2,3 of this row
     uint32_t NEW23 = NEW01 + 0x00020002u;
     uint32_t nact = 0;
+    uint32_t acc_e = 0, acc_n = 0, acc_m = 0;            // byte-wise sums for the fused energy / magnetisation count
     int qn = 0;                                          // queued entries (warp-uniform)
     uint32_t fl = 0;                                     // mismatch flags, 4 per row, the newest row in bits 0..3
     uint32_t fe = 0;                                     // link flags, 1 per row, the newest row in bit 0
@@ -453,7 +468,14 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
             uint32_t wnext = __shfl_down_sync(FULLM, w0, 1);
             if (is_last) wnext = h0;
             const uint32_t east = __funnelshift_r(w0, wnext, 8);
-            G = bond_byte<ISING>(p, d, w0, east, w1);
+            uint32_t ce, cn;
+            G = bond_byte<ISING>(p, d, w0, east, w1, ce, cn);
+            // energy and magnetisation of the configuration this sweep starts from, for free (Eq. 1; BJ north_star (5)):
+            // the (un)satisfied-bond bits are here already; they are added up byte-wise (2 / 4 per bond, at most TH = 32 rows:
+            // no byte overflows) with adds on the multiply-add pipe and evaluated once per strip
+            acc_e = mad_lo(ce, 1u, acc_e);
+            acc_n = mad_lo(cn, 1u, acc_n);
+            if (ISING) acc_m = mad_lo(w0 & 0x02020202u, 1u, acc_m);       // a byte 0xFF (spin -1) adds 2
             c0 += (uint32_t)L >> 1;
             w0 = w1; w1 = w2; w2 = w3; h0 = h1; h1 = h2; h2 = h3;
         } else {
@@ -550,8 +572,19 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
 
     if (!FROM_BONDS) {
         nact = __reduce_add_sync(FULLM, nact);
-        if (lane == 0 && nact)
-            atomicAdd(&acc->part[(tx + 5 * ty) & (ACC_PARTS - 1)].n_active, (unsigned long long)nact);
+        // satisfied bonds of my 4 columns: Ising counts the unsatisfied ones (2 resp. 4 per bond), Potts the satisfied ones
+        uint32_t nsat = (byte_sum(acc_e) >> 1) + (byte_sum(acc_n) >> 2);
+        if (ISING) nsat = 8u * (uint32_t)th_eff - nsat;
+        uint32_t nminus = byte_sum(acc_m) >> 1;
+        if (!colv) nsat = nminus = 0;                    // lanes beyond a ragged edge count nothing
+        nsat = __reduce_add_sync(FULLM, nsat);
+        if (ISING) nminus = __reduce_add_sync(FULLM, nminus);
+        if (lane == 0) {
+            AccPart* const part = &acc->part[(tx + 5 * ty) & (ACC_PARTS - 1)];
+            if (nact) atomicAdd(&part->n_active, (unsigned long long)nact);
+            if (nsat) atomicAdd(&part->sat, (unsigned long long)nsat);
+            if (ISING && nminus) atomicAdd(&part->minus, (unsigned long long)nminus);
+        }
     }
 }
 }  // namespace swb

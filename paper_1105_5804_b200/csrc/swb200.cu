@@ -32,6 +32,8 @@ struct sw_handle {
     int32_t*  d_edgeA;             // (ntx+nty)*L: strip-local roots of last columns / last rows (-1: bond inactive)
     int32_t*  d_edgeB;             // (ntx+nty)*L: strip-local roots of first columns / first rows
     int32_t*  d_size;              // N int32
+    SeriesEntry* d_series;         // SERIES_RING entries: (sat, minus) of the configuration each sweep / step started from
+    uint64_t  series_lo, series_hi; // counters [lo, hi) whose entries are in the ring
     uint32_t* d_draws;             // draw cache: ntx*nty*TH/4*32 words (scan_kernel.cuh)
     bool      draws_valid;         // the cache holds the draws of step draws_t for threshold draws_T
     uint64_t  draws_t;
@@ -51,7 +53,7 @@ namespace {
 constexpr size_t ALIGN = 256;
 inline size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
-struct WorkLayout { size_t acc, wolff, edgeA, edgeB, draws, size, total; };
+struct WorkLayout { size_t acc, wolff, series, edgeA, edgeB, draws, size, total; };
 
 WorkLayout work_layout(int32_t L)
 {
@@ -60,7 +62,8 @@ WorkLayout work_layout(int32_t L)
     WorkLayout w;
     w.acc = 0;
     w.wolff = align_up(sizeof(Acc));
-    w.edgeA = w.wolff + align_up(sizeof(unsigned long long) * WOLFF_RING);
+    w.series = w.wolff + align_up(sizeof(unsigned long long) * WOLFF_RING);
+    w.edgeA = w.series + align_up(sizeof(SeriesEntry) * SERIES_RING);
     w.edgeB = w.edgeA + align_up((ntx + nty) * (size_t)L * sizeof(int32_t));
     w.draws = w.edgeB + align_up((ntx + nty) * (size_t)L * sizeof(int32_t));
     w.size = w.draws + align_up(ntx * nty * (size_t)(TH / 4) * 32 * sizeof(uint32_t));
@@ -135,7 +138,8 @@ inline int grid_capped(int64_t n, int block, int cap) { int g = grid_for(n, bloc
 // labelling of the bond graph of step t (or of packed bonds): k_scan -> k_seam; k_final resolves the rest
 // SRC_PHILOX falls through to SRC_DRAWS when the draw cache holds the draws of step t for the current threshold
 template <int SRC>
-int launch_label_front(sw_handle* h, const Params& p, const uint8_t* bonds, int32_t* labels, cudaStream_t s)
+int launch_label_front(sw_handle* h, const Params& p, const uint8_t* bonds, int32_t* labels, cudaStream_t s,
+                       bool record_series = false)
 {
     SW_PROF(h, 0, s);
     const dim3 grid((p.ntx + SCAN_WARPS - 1) / SCAN_WARPS, p.nty);
@@ -160,8 +164,14 @@ int launch_label_front(sw_handle* h, const Params& p, const uint8_t* bonds, int3
     SW_LAUNCHED(h, "k_scan");
     SW_PROF(h, 1, s);
     const int nseam = (p.ntx + p.nty) * p.L;
-    k_seam<<<grid_for(seam_part(nseam), 256), 256, 0, s>>>(p, h->d_edgeA, h->d_edgeB, labels);
+    k_seam<<<grid_for(seam_part(nseam), 256), 256, 0, s>>>(p, h->d_edgeA, h->d_edgeB, labels, h->d_acc,
+                                                            record_series ? h->d_series : nullptr);
     SW_LAUNCHED(h, "k_seam");
+    if (record_series) {                                 // the ring now holds the entry of counter t
+        if (t != h->series_hi) h->series_lo = t;
+        h->series_hi = t + 1;
+        if (h->series_hi - h->series_lo > (uint64_t)SERIES_RING) h->series_lo = h->series_hi - SERIES_RING;
+    }
     SW_PROF(h, 2, s);
     return SW_OK;
 }
@@ -281,6 +291,8 @@ int sw_bind(sw_handle* h, void* d_spins, int32_t* d_labels, uint8_t* d_bonds, vo
     h->d_edgeB = (int32_t*)(h->d_work + w.edgeB);
     h->d_size = (int32_t*)(h->d_work + w.size);
     h->d_draws = (uint32_t*)(h->d_work + w.draws);
+    h->d_series = (SeriesEntry*)(h->d_work + w.series);
+    h->series_lo = h->series_hi = 0;
     h->draws_valid = false;
     h->bound = false;
     h->last_labels = nullptr;
@@ -314,7 +326,7 @@ int sw_sweep(sw_handle* h, int64_t n, void* stream)
         const Params p = params_at(h, h->t);
         int rc = zero_sweep_counters(h, s);
         if (rc) return rc;
-        rc = launch_label_front<SRC_PHILOX>(h, p, nullptr, h->d_labels, s);
+        rc = launch_label_front<SRC_PHILOX>(h, p, nullptr, h->d_labels, s, true);
         if (rc) return rc;
         // the flatten + flip pass also draws the bonds of step t+1 (draw cache): the next sweep's k_scan only reads them
         {
@@ -416,7 +428,7 @@ int wolff_step(sw_handle* h, int64_t n, int64_t* h_sizes, void* stream)
             const Params p = params_at(h, h->t);
             int rc = zero_sweep_counters(h, s);
             if (rc) return rc;
-            rc = launch_label_front<SRC_PHILOX>(h, p, nullptr, h->d_labels, s);
+            rc = launch_label_front<SRC_PHILOX>(h, p, nullptr, h->d_labels, s, true);
             if (rc) return rc;
             if ((p.L % TW) == 0 && (p.L % TH) == 0)
                 k_final<MODE_WOLFF, 0, true, true><<<dim3(p.ntx, p.nty), FIN_THREADS, 0, s>>>(p, h->d_labels, h->d_spins,
@@ -493,6 +505,32 @@ int sw_observables_ex(sw_handle* h, sw_obs* h_out, int flags, void* stream)
 int sw_observables(sw_handle* h, sw_obs* h_out, void* stream)
 {
     return sw_observables_ex(h, h_out, SW_OBS_SPINS | SW_OBS_CLUSTERS, stream);
+}
+
+int sw_series_read(sw_handle* h, uint64_t t_first, int64_t n, int64_t* h_energy, int64_t* h_magnetisation, void* stream)
+{
+    if (!h || n < 0 || (n > 0 && !h_energy) || (h->q != 2 && h_magnetisation)) return SW_EINVAL;
+    if (!h->bound) return SW_ESTATE;
+    if (n == 0) return SW_OK;
+    if (t_first < h->series_lo || t_first + (uint64_t)n > h->series_hi) return SW_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    SeriesEntry* buf = new (std::nothrow) SeriesEntry[(size_t)n];
+    if (!buf) return SW_ENOMEM;
+    const uint64_t i0 = t_first & (SERIES_RING - 1);
+    const uint64_t n1 = (uint64_t)n < SERIES_RING - i0 ? (uint64_t)n : SERIES_RING - i0;      // up to the end of the ring
+    cudaError_t e = cudaMemcpyAsync(buf, h->d_series + i0, sizeof(SeriesEntry) * n1, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess && n1 < (uint64_t)n)
+        e = cudaMemcpyAsync(buf + n1, h->d_series, sizeof(SeriesEntry) * ((uint64_t)n - n1), cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) { delete[] buf; return cuda_fail(h, e, "sw_series_read"); }
+    const int64_t N = h->N;
+    for (int64_t k = 0; k < n; ++k) {
+        const int64_t sat = (int64_t)buf[k].sat;
+        h_energy[k] = h->q == 2 ? -(2 * sat - 2 * N) : -sat;
+        if (h_magnetisation) h_magnetisation[k] = N - 2 * (int64_t)buf[k].minus;
+    }
+    delete[] buf;
+    return SW_OK;
 }
 
 int sw_sweep_host(sw_handle* h, const void* h_spins_in, int64_t n, void* h_spins_out, int32_t* h_labels_out,

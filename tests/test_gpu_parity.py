@@ -247,3 +247,57 @@ def test_sweep_host_end_to_end():
     assert np.array_equal(h_out.numpy(), s) and np.array_equal(h_lab.numpy(), lab)
     assert o["energy"] == oracle.observables(L, 2, s)["energy"] and o["n_clusters"] == nc
     lat.close()
+
+
+# ------------------------------------------------------------------------------------------------ fused E / M series
+@pytest.mark.parametrize("L,q,beta,mode", [(64, 2, BETA_C, 1), (132, 2, 0.5, 0), (260, 2, 0.4, 1), (96, 3, oracle.beta_c(3), 1)])
+def test_series_of_a_chain_matches_the_oracle(L, q, beta, mode):
+    """sw_series_read: E (and M for q=2) of the configuration every sweep started from, counted by the sweep's own scan
+    kernel, against the oracle's observables of the same chain -- bit for bit, including ragged strips (L=132, 260)."""
+    seed, n = 21, 37
+    lat = binding.Lattice(L, q, beta, seed)
+    lat.init_spins(mode)
+    s = oracle.init_spins(L, q, seed, mode)
+    T = lat.get_threshold()
+    want_E, want_M = [], []
+    for t in range(n):
+        w = oracle.observables(L, q, s)
+        want_E.append(w["energy"]); want_M.append(w["magnetisation"])
+        oracle.sweep(L, q, T, seed, t, s)
+    lat.sweep(10)
+    lat.sweep(n - 10)                                      # two batched calls: the series is contiguous across calls
+    E, M = lat.series(0, n, magnetisation=(q == 2))
+    assert E == want_E
+    if q == 2:
+        assert M == want_M
+    else:
+        with pytest.raises(binding.SwError):
+            lat.series(0, n, magnetisation=True)
+    assert lat.series(n - 5, 5, magnetisation=False)[0] == want_E[-5:]
+    with pytest.raises(binding.SwError):
+        lat.series(0, n + 1, magnetisation=False)          # the current configuration has not been scanned yet
+    # the state is untouched: spins equal the oracle's
+    assert np.array_equal(lat.spins_host(), s)
+    lat.close()
+
+
+def test_series_ring_wraps_and_follows_wolff_steps():
+    L, seed = 8, 5
+    lat = binding.Lattice(L, 2, BETA_C, seed)
+    lat.init_spins(1)
+    s = oracle.init_spins(L, 2, seed, 1)
+    T = lat.get_threshold()
+    n = 4096 + 300                                         # more sweeps than the ring holds
+    ser = oracle.run_chain(L, 2, T, seed, 0, n, s)         # (E, M, ...) AFTER every sweep = configuration at counter t+1
+    lat.sweep(n)
+    E, M = lat.series(n - 4096, 4096)
+    assert E == [int(x) for x in ser[n - 4097:n - 1, 0]] and M == [int(x) for x in ser[n - 4097:n - 1, 1]]
+    with pytest.raises(binding.SwError):
+        lat.series(n - 4097, 4)                            # overwritten
+    # Wolff steps are filed under their counters too
+    w = oracle.wolff_chain(L, T, seed, n, 6, s)
+    lat.wolff_step(6)
+    E, M = lat.series(n, 6)
+    assert E == [int(ser[n - 1, 0])] + [int(x) for x in w[:5, 0]]
+    assert M == [int(ser[n - 1, 1])] + [int(x) for x in w[:5, 1]]
+    lat.close()
