@@ -128,6 +128,15 @@ int sw_cluster_stats(sw_handle* h, const int32_t* d_labels_in, sw_cstats* h_out,
  * step -- in that case the call synchronises `stream` before returning. */
 int wolff_step(sw_handle* h, int64_t n, int64_t* h_sizes, void* stream);
 
+/* Frontier growth for wolff_step (P:355 option (b); S:8f.1).  max_levels = 0 (default): every step decomposes the whole
+ * lattice and flips one cluster.  max_levels > 0: a step first grows the cluster from the seed site level by level --
+ * the bond draws are pure functions of (seed, t, site, direction), so it is the same cluster, and only the bonds that
+ * are looked at are drawn; if the frontier is not empty after max_levels levels the spins are restored and the step is
+ * done by the labelling path after all.  A level costs about 2 microseconds whatever its width, so this pays for small
+ * clusters only (beta < beta_c; at beta_c the median Wolff cluster of a large lattice has ~10^5..10^6 sites).  In this
+ * mode wolff_step maintains neither d_labels nor the energy series, and the cluster part of sw_obs is zero. */
+int sw_wolff_frontier(sw_handle* h, int max_levels);
+
 /* Energy, magnetisation, state counts of the current spins and cluster statistics of the last labelling, all in
  * int64 (S:8a a6).  Synchronises `stream`.  Equals sw_observables_ex(.., SW_OBS_SPINS | SW_OBS_CLUSTERS, ..). */
 int sw_observables(sw_handle* h, sw_obs* h_out, void* stream);

@@ -20,7 +20,7 @@ NPHASE = 3                                                # SW_NPHASE of include
 SYMBOLS = [
     "sw_create", "sw_destroy", "sw_workspace_bytes", "sw_bind", "sw_set_threshold", "sw_get_threshold",
     "sw_set_counter", "sw_get_counter", "sw_init_spins", "sw_sweep", "sw_activate", "sw_label",
-    "sw_cluster_stats", "wolff_step", "sw_observables", "sw_observables_ex", "sw_series_read", "sw_sweep_host", "sw_launch_count", "sw_strerror",
+    "sw_cluster_stats", "wolff_step", "sw_observables", "sw_observables_ex", "sw_series_read", "sw_wolff_frontier", "sw_sweep_host", "sw_launch_count", "sw_strerror",
     "sw_last_cuda_error", "sw_profile_enable", "sw_profile_read",
 ]
 
@@ -76,6 +76,7 @@ def lib():
     L.wolff_step.argtypes = [vp, i64, C.POINTER(i64), vp]
     L.sw_observables.argtypes = [vp, C.POINTER(sw_obs), vp]
     L.sw_observables_ex.argtypes = [vp, C.POINTER(sw_obs), C.c_int, vp]
+    L.sw_wolff_frontier.argtypes = [vp, C.c_int]
     L.sw_series_read.argtypes = [vp, u64, i64, C.POINTER(i64), C.POINTER(i64), vp]
     L.sw_sweep_host.argtypes = [vp, vp, i64, vp, vp, C.POINTER(sw_obs), vp]
     L.sw_launch_count.argtypes = [vp, C.POINTER(u64)]
@@ -186,6 +187,9 @@ class Lattice:
             return list(sizes)
         self._check(self._lib.wolff_step(self._h, n, None, self._stream()))
         return None
+
+    def wolff_frontier(self, max_levels: int):
+        self._check(self._lib.sw_wolff_frontier(self._h, max_levels))
 
     def observables(self, spins: bool = True, clusters: bool = True) -> dict:
         out = sw_obs()

@@ -10,6 +10,7 @@
 #include "common.cuh"
 #include "label_kernels.cuh"
 #include "misc_kernels.cuh"
+#include "wolff_kernel.cuh"
 
 using namespace swb;
 
@@ -35,6 +36,8 @@ struct sw_handle {
     SeriesEntry* d_series;         // SERIES_RING entries: (sat, minus) of the configuration each sweep / step started from
     uint64_t  series_lo, series_hi; // counters [lo, hi) whose entries are in the ring
     uint32_t* d_draws;             // draw cache: ntx*nty*TH/4*32 words (scan_kernel.cuh)
+    int       wolff_levels;        // 0: label everything; > 0: try frontier growth for that many levels first
+    int*      d_wolff_status;      // device flag of the frontier kernel (0 done, 1 gave up)
     bool      draws_valid;         // the cache holds the draws of step draws_t for threshold draws_T
     uint64_t  draws_t;
     uint32_t  draws_T;
@@ -53,7 +56,7 @@ namespace {
 constexpr size_t ALIGN = 256;
 inline size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
-struct WorkLayout { size_t acc, wolff, series, edgeA, edgeB, draws, size, total; };
+struct WorkLayout { size_t acc, wolff, wstatus, series, edgeA, edgeB, draws, size, total; };
 
 WorkLayout work_layout(int32_t L)
 {
@@ -62,7 +65,8 @@ WorkLayout work_layout(int32_t L)
     WorkLayout w;
     w.acc = 0;
     w.wolff = align_up(sizeof(Acc));
-    w.series = w.wolff + align_up(sizeof(unsigned long long) * WOLFF_RING);
+    w.wstatus = w.wolff + align_up(sizeof(unsigned long long) * WOLFF_RING);
+    w.series = w.wstatus + align_up(sizeof(int));
     w.edgeA = w.series + align_up(sizeof(SeriesEntry) * SERIES_RING);
     w.edgeB = w.edgeA + align_up((ntx + nty) * (size_t)L * sizeof(int32_t));
     w.draws = w.edgeB + align_up((ntx + nty) * (size_t)L * sizeof(int32_t));
@@ -292,6 +296,7 @@ int sw_bind(sw_handle* h, void* d_spins, int32_t* d_labels, uint8_t* d_bonds, vo
     h->d_size = (int32_t*)(h->d_work + w.size);
     h->d_draws = (uint32_t*)(h->d_work + w.draws);
     h->d_series = (SeriesEntry*)(h->d_work + w.series);
+    h->d_wolff_status = (int*)(h->d_work + w.wstatus);
     h->series_lo = h->series_hi = 0;
     h->draws_valid = false;
     h->bound = false;
@@ -414,33 +419,64 @@ int sw_cluster_stats(sw_handle* h, const int32_t* d_labels_in, sw_cstats* h_out,
     return SW_OK;
 }
 
+// one Wolff step by "decompose everything, flip one cluster"; |C| is added to *d_size_slot (zeroed by the caller)
+static int wolff_step_labelling(sw_handle* h, unsigned long long* d_size_slot, bool maintain, cudaStream_t s)
+{
+    const Params p = params_at(h, h->t);
+    int rc = zero_sweep_counters(h, s);
+    if (rc) return rc;
+    rc = launch_label_front<SRC_PHILOX>(h, p, nullptr, h->d_labels, s, maintain);
+    if (rc) return rc;
+    if ((p.L % TW) == 0 && (p.L % TH) == 0)
+        k_final<MODE_WOLFF, 0, true, true><<<dim3(p.ntx, p.nty), FIN_THREADS, 0, s>>>(p, h->d_labels, h->d_spins, h->d_acc,
+                                                                                    d_size_slot, nullptr);
+    else
+        k_final<MODE_WOLFF, 0, false, true><<<dim3(p.ntx, p.nty), FIN_THREADS, 0, s>>>(p, h->d_labels, h->d_spins, h->d_acc,
+                                                                                     d_size_slot, nullptr);
+    SW_LAUNCHED(h, "k_final<WOLFF>");
+    SW_PROF(h, 3, s);
+    if (h->prof_on && h->prof_n < PROF_MAX) ++h->prof_n;
+    ++h->t;
+    return SW_OK;
+}
+
 int wolff_step(sw_handle* h, int64_t n, int64_t* h_sizes, void* stream)
 {
     if (!h || n < 0) return SW_EINVAL;
     if (h->q != 2) return SW_EINVAL;                     // DESIGN.md reading 8: the paper defines Wolff for Ising only
     if (!h->bound) return SW_ESTATE;
     cudaStream_t s = (cudaStream_t)stream;
+    const bool front = h->wolff_levels > 0;
     int64_t done = 0;
     while (done < n) {
         const int64_t batch = (n - done) < WOLFF_RING ? (n - done) : WOLFF_RING;
         SW_CUDA(h, cudaMemsetAsync(h->d_wolff, 0, sizeof(unsigned long long) * (size_t)batch, s));
-        for (int64_t k = 0; k < batch; ++k) {
-            const Params p = params_at(h, h->t);
-            int rc = zero_sweep_counters(h, s);
-            if (rc) return rc;
-            rc = launch_label_front<SRC_PHILOX>(h, p, nullptr, h->d_labels, s, true);
-            if (rc) return rc;
-            if ((p.L % TW) == 0 && (p.L % TH) == 0)
-                k_final<MODE_WOLFF, 0, true, true><<<dim3(p.ntx, p.nty), FIN_THREADS, 0, s>>>(p, h->d_labels, h->d_spins,
-                                                                                            h->d_acc, h->d_wolff + k, nullptr);
-            else
-                k_final<MODE_WOLFF, 0, false, true><<<dim3(p.ntx, p.nty), FIN_THREADS, 0, s>>>(p, h->d_labels, h->d_spins,
-                                                                                             h->d_acc, h->d_wolff + k, nullptr);
-            SW_LAUNCHED(h, "k_final<WOLFF>");
-            SW_PROF(h, 3, s);
-            if (h->prof_on && h->prof_n < PROF_MAX) ++h->prof_n;
-            ++h->t;
-            h->last_labels = h->d_labels;
+        int64_t k = 0;
+        while (k < batch) {
+            if (!front) {
+                int rc = wolff_step_labelling(h, h->d_wolff + k, true, s);
+                if (rc) return rc;
+                h->last_labels = h->d_labels;
+                ++k;
+                continue;
+            }
+            // frontier growth (wolff_kernel.cuh): as many steps as finish within the level budget, in one launch
+            k_wolff_front<<<1, WOLFF_THREADS, 0, s>>>(params_at(h, h->t), h->d_spins, h->d_size, h->wolff_levels,
+                                                      (int)(batch - k), h->d_wolff + k, h->d_wolff_status);
+            SW_LAUNCHED(h, "k_wolff_front");
+            int ndone = 0;
+            SW_CUDA(h, cudaMemcpyAsync(&ndone, h->d_wolff_status, sizeof(int), cudaMemcpyDeviceToHost, s));
+            SW_CUDA(h, cudaStreamSynchronize(s));
+            h->t += (uint64_t)ndone;
+            k += ndone;
+            if (k < batch) {                             // the step at counter t was given up (spins restored): label everything
+                int rc = wolff_step_labelling(h, h->d_wolff + k, false, s);
+                if (rc) return rc;
+                ++k;
+            }
+            // in this mode the labels buffer and the series are not maintained (most steps label nothing)
+            h->last_labels = nullptr;
+            h->series_lo = h->series_hi = h->t;
         }
         if (h_sizes) {
             SW_CUDA(h, cudaMemcpyAsync(h_sizes + done, h->d_wolff, sizeof(int64_t) * (size_t)batch,
@@ -449,6 +485,13 @@ int wolff_step(sw_handle* h, int64_t n, int64_t* h_sizes, void* stream)
         }
         done += batch;
     }
+    return SW_OK;
+}
+
+int sw_wolff_frontier(sw_handle* h, int max_levels)
+{
+    if (!h || max_levels < 0) return SW_EINVAL;
+    h->wolff_levels = max_levels;
     return SW_OK;
 }
 

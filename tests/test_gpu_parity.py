@@ -301,3 +301,36 @@ def test_series_ring_wraps_and_follows_wolff_steps():
     assert E == [int(ser[n - 1, 0])] + [int(x) for x in w[:5, 0]]
     assert M == [int(ser[n - 1, 1])] + [int(x) for x in w[:5, 1]]
     lat.close()
+
+
+# ------------------------------------------------------------------------------------------------ frontier Wolff
+@pytest.mark.parametrize("L,beta,levels,nsteps", [(64, BETA_C, 1000, 60), (64, BETA_C, 2, 60), (256, 0.40, 40, 80),
+                                                  (132, 0.30, 1000, 50), (4, BETA_C, 5, 50), (256, 0.5, 3, 25)])
+def test_wolff_frontier_growth_matches_the_oracle(L, beta, levels, nsteps):
+    """sw_wolff_frontier: the cluster grown from the seed site (bonds drawn on demand) must be the oracle's cluster --
+    sizes and spins after every step -- whether the growth finishes (large `levels`) or gives up and hands the step to the
+    labelling path (small `levels`: clusters deeper than that take the fallback, spins restored first)."""
+    seed = 77
+    lat = binding.Lattice(L, 2, beta, seed)
+    T = lat.get_threshold()
+    lat.init_spins(1)
+    lat.sweep(5)
+    s = lat.spins_host().copy()
+    t0 = lat.get_counter()
+    lat.wolff_frontier(levels)
+    for k in range(nsteps):
+        sizes = lat.wolff_step(1)
+        sz, i0, root = oracle.wolff_step(L, T, seed, t0 + k, s)
+        assert sizes == [sz], k
+        assert np.array_equal(lat.spins_host(), s), k
+    sizes = lat.wolff_step(9)                              # a batch call equals single calls
+    want = [oracle.wolff_step(L, T, seed, t0 + nsteps + k, s)[0] for k in range(9)]
+    assert sizes == want and np.array_equal(lat.spins_host(), s)
+    o = lat.observables()
+    assert o["n_clusters"] == 0 and o["counter"] == t0 + nsteps + 9      # no labelling is maintained in this mode
+    # back to the labelling path: labels and series are maintained again
+    lat.wolff_frontier(0)
+    sizes = lat.wolff_step(1)
+    sz, i0, root = oracle.wolff_step(L, T, seed, t0 + nsteps + 9, s)
+    assert sizes == [sz] and lat.labels_host()[i0] == root and np.array_equal(lat.spins_host(), s)
+    lat.close()
