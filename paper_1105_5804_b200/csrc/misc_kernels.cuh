@@ -65,21 +65,43 @@ __device__ __forceinline__ unsigned long long warp_sum_u64(unsigned long long v)
 __global__ void __launch_bounds__(256)
 k_observables(const Params p, const uint32_t* __restrict__ spins_w, Acc* __restrict__ acc)
 {
-    const int L = p.L, Lw = L >> 2, nw = p.N >> 2;
+    const int L = p.L, Lw = L >> 2;
     unsigned long long sat = 0, cnt[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-    for (int i4 = blockIdx.x * blockDim.x + threadIdx.x; i4 < nw; i4 += gridDim.x * blockDim.x) {
-        const int yy = i4 / Lw, xw = i4 - yy * Lw;
-        const uint32_t w = spins_w[i4];
-        const uint32_t we = spins_w[yy * Lw + (xw + 1 == Lw ? 0 : xw + 1)];
-        const uint32_t wn = spins_w[(yy + 1 == L ? 0 : yy + 1) * Lw + xw];
-        sat += __popc(eq_bytes4(w, __funnelshift_r(w, we, 8))) + __popc(eq_bytes4(w, wn));
-        if (p.q == 2) {
-            cnt[1] += __popc(w & 0x80808080u);           // bytes equal to -1
-        } else {
+    // a CTA takes a block of consecutive rows (no index division; the north row of one iteration is the row of the next and
+    // comes from the cache); the east word is the next word of the row (periodic)
+    const int rows_per = (L + gridDim.x - 1) / gridDim.x;
+    const int y_begin = blockIdx.x * rows_per, y_end = min(L, y_begin + rows_per);
+    for (int yy = y_begin; yy < y_end; ++yy) {
+        const uint32_t* const row = spins_w + (size_t)yy * Lw;
+        const uint32_t* const nrow = spins_w + (size_t)(yy + 1 == L ? 0 : yy + 1) * Lw;
+        uint32_t s = 0, c = 0;
+        auto word = [&](uint32_t w, uint32_t we, uint32_t wn) {
+            const uint32_t east = __funnelshift_r(w, we, 8);
+            if (p.q == 2) {                              // bytes 0x01 / 0xFF: bit 1 (2) of the xor is set iff the spins differ
+                s += 8 - __popc(((w ^ east) & 0x02020202u) | ((w ^ wn) & 0x04040404u));
+                c += __popc(w & 0x80808080u);            // bytes equal to -1
+            } else {
+                s += __popc(eq_bytes4(w, east)) + __popc(eq_bytes4(w, wn));
 #pragma unroll
-            for (int k = 1; k < 8; ++k)
-                if (k < p.q) cnt[k] += __popc(__vcmpeq4(w, 0x01010101u * k) & 0x01010101u);
+                for (int k = 1; k < 8; ++k)
+                    if (k < p.q) cnt[k] += __popc(__vcmpeq4(w, 0x01010101u * k) & 0x01010101u);
+            }
+        };
+        if ((Lw & 3) == 0) {                             // 128-bit loads: 16 sites per thread and iteration
+            const int Lv = Lw >> 2;
+#pragma unroll 2
+            for (int xv = threadIdx.x; xv < Lv; xv += blockDim.x) {
+                const uint4 v = reinterpret_cast<const uint4*>(row)[xv];
+                const uint4 vn = reinterpret_cast<const uint4*>(nrow)[xv];
+                const uint32_t e = row[xv + 1 == Lv ? 0 : 4 * xv + 4];
+                word(v.x, v.y, vn.x); word(v.y, v.z, vn.y); word(v.z, v.w, vn.z); word(v.w, e, vn.w);
+            }
+        } else {
+            for (int xw = threadIdx.x; xw < Lw; xw += blockDim.x)
+                word(row[xw], row[xw + 1 == Lw ? 0 : xw + 1], nrow[xw]);
         }
+        sat += s;
+        cnt[1] += c;
     }
     sat = warp_sum_u64(sat);
 #pragma unroll

@@ -503,7 +503,7 @@ int sw_observables_ex(sw_handle* h, sw_obs* h_out, int flags, void* stream)
     const Params p = params_at(h, h->t);
     if (flags & SW_OBS_SPINS) {
         SW_CUDA(h, cudaMemsetAsync(&h->d_acc->sat, 0, sizeof(unsigned long long) * 9, s));
-        k_observables<<<grid_capped(h->N / 4, 256, 148 * 8), 256, 0, s>>>(p, h->d_spins, h->d_acc);
+        k_observables<<<(h->L < 148 * 8 ? h->L : 148 * 8), 256, 0, s>>>(p, h->d_spins, h->d_acc);
         SW_LAUNCHED(h, "k_observables");
     }
     const bool clusters = (flags & SW_OBS_CLUSTERS) && h->last_labels;
