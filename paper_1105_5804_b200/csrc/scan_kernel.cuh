@@ -306,30 +306,32 @@ __device__ __forceinline__ void unite_batch(volatile uint16_t* nm, bool have, ui
 __device__ __forceinline__ void drain_flags(uint32_t flags, int sh, int pos0, uint32_t tag, volatile uint16_t* q, int& qn,
                                             volatile uint16_t* nm, int* prov, int base, int L, int lane, unsigned lt)
 {
-    const int cnt = __popc(flags);
-    int incl = cnt;
+    if (SWB_DRAIN_SCAN && QCAP >= 128) {                 // (a 64-entry queue never takes 8 rows at once: skip the scan)
+        const int cnt = __popc(flags);
+        int incl = cnt;
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const int t = __shfl_up_sync(FULLM, incl, o);
-        if (lane >= o) incl += t;
-    }
-    const int total = __shfl_sync(FULLM, incl, 31);
-    if (total == 0) return;
-    if (SWB_DRAIN_SCAN && total <= QCAP - qn) {
-        volatile uint16_t* out = q + qn + (incl - cnt);
-        while (flags) {
-            const int b = 31 - __clz(flags);
-            flags ^= 1u << b;
-            *out++ = (uint16_t)((uint32_t)(pos0 - ((b >> sh) << TW_LOG) + (b & ((1 << sh) - 1))) | tag);
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(FULLM, incl, o);
+            if (lane >= o) incl += t;
         }
-        qn += total;
-        __syncwarp();                                    // queue entries and forest rows visible to the whole warp
-        while (qn >= 32) {
-            qn -= 32;
-            unite_batch(nm, true, q[qn + lane], prov, base, L);
+        const int total = __shfl_sync(FULLM, incl, 31);
+        if (total == 0) return;
+        if (total <= QCAP - qn) {
+            volatile uint16_t* out = q + qn + (incl - cnt);
+            while (flags) {
+                const int b = 31 - __clz(flags);
+                flags ^= 1u << b;
+                *out++ = (uint16_t)((uint32_t)(pos0 - ((b >> sh) << TW_LOG) + (b & ((1 << sh) - 1))) | tag);
+            }
+            qn += total;
+            __syncwarp();                                // queue entries and forest rows visible to the whole warp
+            while (qn >= 32) {
+                qn -= 32;
+                unite_batch(nm, true, q[qn + lane], prov, base, L);
+            }
+            __syncwarp();                                // queue slots read before they are overwritten
+            return;
         }
-        __syncwarp();                                    // queue slots read before they are overwritten
-        return;
     }
     while (true) {
         const bool has = flags != 0u;
