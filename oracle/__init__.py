@@ -105,6 +105,21 @@ def lib():
         L.orc_wolff_chain.restype = C.c_int
         L.orc_fnv1a64.argtypes = [pu8, C.c_int64]
         L.orc_fnv1a64.restype = C.c_uint64
+        # simple cubic lattice
+        L.orc3_init_spins.argtypes = [C.c_int32, C.c_int32, C.c_uint64, C.c_int32, p8]
+        L.orc3_init_spins.restype = C.c_int
+        L.orc3_bonds.argtypes = [C.c_int32, C.c_uint32, C.c_uint64, C.c_uint64, p8, pu8]
+        L.orc3_bonds.restype = C.c_int64
+        L.orc3_label.argtypes = [C.c_int32, pu8, p32]
+        L.orc3_label.restype = C.c_int64
+        L.orc3_flip.argtypes = [C.c_int64, C.c_int32, C.c_uint64, C.c_uint64, p32, p8]
+        L.orc3_flip.restype = None
+        L.orc3_observables.argtypes = [C.c_int32, C.c_int32, p8, C.POINTER(Obs)]
+        L.orc3_observables.restype = None
+        L.orc3_sweep.argtypes = [C.c_int32, C.c_int32, C.c_uint32, C.c_uint64, C.c_uint64, p8, p32, pu8, p64]
+        L.orc3_sweep.restype = C.c_int64
+        L.orc3_run_chain.argtypes = [C.c_int32, C.c_int32, C.c_uint32, C.c_uint64, C.c_uint64, C.c_int64, p8, p64]
+        L.orc3_run_chain.restype = C.c_int
         _lib = L
     return _lib
 
@@ -244,3 +259,63 @@ def wolff_chain(L: int, T: int, seed: int, t0: int, n: int, spins: np.ndarray) -
 def fnv1a64(buf: np.ndarray) -> int:
     b = np.ascontiguousarray(buf).view(np.uint8).reshape(-1)
     return int(lib().orc_fnv1a64(_p(b, C.c_uint8), b.size))
+
+
+# ---- simple cubic lattice: site i = z L^2 + y L + x, bond codes bit 0 east, 1 north, 2 up ----------
+def init_spins3(L: int, q: int, seed: int, mode: int) -> np.ndarray:
+    s = np.empty(L ** 3, dtype=np.int8)
+    if lib().orc3_init_spins(L, q, seed, mode, _p(s, C.c_int8)) != 0:
+        raise ValueError("orc3_init_spins: bad arguments")
+    return s
+
+
+def bonds3(L: int, T: int, seed: int, t: int, spins: np.ndarray):
+    assert spins.dtype == np.int8 and spins.size == L ** 3 and spins.flags.c_contiguous
+    codes = np.empty(L ** 3, dtype=np.uint8)
+    n = lib().orc3_bonds(L, T, seed, t, _p(spins, C.c_int8), _p(codes, C.c_uint8))
+    return codes, int(n)
+
+
+def label3(L: int, codes: np.ndarray):
+    codes = np.ascontiguousarray(codes, dtype=np.uint8)
+    assert codes.size == L ** 3
+    labels = np.empty(L ** 3, dtype=np.int32)
+    nc = lib().orc3_label(L, _p(codes, C.c_uint8), _p(labels, C.c_int32))
+    if nc < 0:
+        raise MemoryError
+    return labels, int(nc)
+
+
+def flip3(q: int, seed: int, t: int, labels: np.ndarray) -> np.ndarray:
+    labels = np.ascontiguousarray(labels, dtype=np.int32)
+    spins = np.empty(labels.size, dtype=np.int8)
+    lib().orc3_flip(labels.size, q, seed, t, _p(labels, C.c_int32), _p(spins, C.c_int8))
+    return spins
+
+
+def observables3(L: int, q: int, spins: np.ndarray) -> dict:
+    assert spins.dtype == np.int8 and spins.size == L ** 3 and spins.flags.c_contiguous
+    o = Obs()
+    lib().orc3_observables(L, q, _p(spins, C.c_int8), C.byref(o))
+    return {"sat_bonds": o.sat_bonds, "energy": o.energy, "magnetisation": o.magnetisation,
+            "state_count": list(o.state_count)}
+
+
+def sweep3(L: int, q: int, T: int, seed: int, t: int, spins: np.ndarray):
+    """One SW sweep of the L^3 lattice in place. -> (labels, codes, n_clusters, n_active_bonds)"""
+    assert spins.dtype == np.int8 and spins.size == L ** 3 and spins.flags.c_contiguous
+    labels = np.empty(L ** 3, dtype=np.int32)
+    codes = np.empty(L ** 3, dtype=np.uint8)
+    nb = C.c_int64(0)
+    nc = lib().orc3_sweep(L, q, T, seed, t, _p(spins, C.c_int8), _p(labels, C.c_int32), _p(codes, C.c_uint8), C.byref(nb))
+    if nc < 0:
+        raise MemoryError
+    return labels, codes, int(nc), int(nb.value)
+
+
+def run_chain3(L: int, q: int, T: int, seed: int, t0: int, n: int, spins: np.ndarray) -> np.ndarray:
+    assert spins.dtype == np.int8 and spins.size == L ** 3 and spins.flags.c_contiguous
+    series = np.zeros((n, 4), dtype=np.int64)
+    if lib().orc3_run_chain(L, q, T, seed, t0, n, _p(spins, C.c_int8), _p(series, C.c_int64)) != 0:
+        raise MemoryError
+    return series

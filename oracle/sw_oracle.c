@@ -391,3 +391,172 @@ uint64_t orc_fnv1a64(const uint8_t *p, int64_t n)
     for (int64_t i = 0; i < n; ++i) { h ^= p[i]; h *= 0x100000001b3ull; }
     return h;
 }
+
+/* ==================================================================================
+ * Simple cubic lattice ("hypercubic lattices", P:154
+ * "three out of six neighbours" are looked after by every site in 3D).  The same
+ * three steps on a periodic L x L x L lattice, site i = z L^2 + y L + x,
+ * each site owning its bonds to the east (x+1), north (y+1) and up (z+1) neighbour.
+ * DESIGN.md reading 19 (the survey fixes the draws for two directions only):
+ *   u3(i,d,t) = PHILOX(seed; i, t_lo, t_hi, BOND3)[d],  d = 0 east, 1 north, 2 up,
+ * one call per site, word 3 unused, domain BOND3 = 4.  Initialisation, threshold and
+ * flip are the 2D definitions over N = L^3 sites (S:8c.4, 8c.6, 8c.8).
+ *
+ * Pins (tests/test_oracle_cubic.py): orc3_bonds -- T = 0 / T = max, never joins
+ * unequal spins, the three directions hit the three distinct neighbours (single-spin
+ * patterns), density; orc3_label -- random bond sets on 3^3 .. 6^3 against an
+ * independent transitive closure and scipy's connected components, wrap bonds in all
+ * three directions; orc3_observables -- numpy definition, closed forms (cold, layered);
+ * orc3_sweep / orc3_run_chain -- exact <E>, <|m|>, <m^2> of the 3 x 3 x 3 Ising model
+ * (sum over all 2^27 states, done plane by plane in the test) and the FK identity.
+ * ================================================================================== */
+enum { DOM_BOND3 = 4 };
+
+static void nbrs3(int64_t L, int64_t i, int64_t nb[6])   /* east, north, up, west, south, down */
+{
+    int64_t x = i % L, y = (i / L) % L, z = i / (L * L);
+    nb[0] = z * L * L + y * L + (x + 1) % L;
+    nb[1] = z * L * L + ((y + 1) % L) * L + x;
+    nb[2] = ((z + 1) % L) * L * L + y * L + x;
+    nb[3] = z * L * L + y * L + (x + L - 1) % L;
+    nb[4] = z * L * L + ((y + L - 1) % L) * L + x;
+    nb[5] = ((z + L - 1) % L) * L * L + y * L + x;
+}
+
+int orc3_init_spins(int32_t L, int32_t q, uint64_t seed, int32_t mode, int8_t *spins)
+{
+    int64_t N = (int64_t)L * L * L;
+    if (L < 3 || q < 2 || q > 8) return -1;
+    for (int64_t i = 0; i < N; ++i) {
+        uint32_t k = 0;
+        if (mode == 1) {
+            uint32_t w[4];
+            draw(seed, (uint32_t)(i >> 2), 0, DOM_INIT, w);
+            k = mulhi_range(w[i & 3], (uint32_t)q);
+        }
+        spins[i] = store_of(q, k);
+    }
+    return 0;
+}
+
+/* codes[i]: bit 0 east, bit 1 north, bit 2 up.  Returns the number of active bonds. */
+int64_t orc3_bonds(int32_t L, uint32_t T, uint64_t seed, uint64_t t, const int8_t *spins, uint8_t *codes)
+{
+    int64_t N = (int64_t)L * L * L, active = 0;
+    for (int64_t i = 0; i < N; ++i) {
+        uint32_t w[4];
+        int64_t nb[6];
+        draw(seed, (uint32_t)i, t, DOM_BOND3, w);
+        nbrs3(L, i, nb);
+        uint8_t c = 0;
+        for (int d = 0; d < 3; ++d)
+            if (spins[i] == spins[nb[d]] && w[d] < T) { c |= (uint8_t)(1u << d); ++active; }
+        codes[i] = c;
+    }
+    return active;
+}
+
+/* breadth-first search, seeds in increasing order: label = minimum site index */
+int64_t orc3_label(int32_t L, const uint8_t *codes, int32_t *labels)
+{
+    int64_t N = (int64_t)L * L * L, nclusters = 0;
+    int32_t *queue = (int32_t *)malloc((size_t)N * sizeof(int32_t));
+    if (!queue) return -1;
+    for (int64_t i = 0; i < N; ++i) labels[i] = -1;
+    for (int64_t seed_site = 0; seed_site < N; ++seed_site) {
+        if (labels[seed_site] != -1) continue;
+        ++nclusters;
+        int64_t head = 0, tail = 0;
+        labels[seed_site] = (int32_t)seed_site;
+        queue[tail++] = (int32_t)seed_site;
+        while (head < tail) {
+            int64_t i = queue[head++], nb[6];
+            nbrs3(L, i, nb);
+            for (int d = 0; d < 3; ++d) {
+                /* my own bond in direction d, and the bond of the neighbour behind me in direction d */
+                if ((codes[i] >> d) & 1) {
+                    int64_t j = nb[d];
+                    if (labels[j] == -1) { labels[j] = (int32_t)seed_site; queue[tail++] = (int32_t)j; }
+                }
+                int64_t j = nb[3 + d];
+                if (((codes[j] >> d) & 1) && labels[j] == -1) { labels[j] = (int32_t)seed_site; queue[tail++] = (int32_t)j; }
+            }
+        }
+    }
+    free(queue);
+    return nclusters;
+}
+
+void orc3_flip(int64_t N, int32_t q, uint64_t seed, uint64_t t, const int32_t *labels, int8_t *spins)
+{
+    for (int64_t i = 0; i < N; ++i) {
+        uint32_t w[4];
+        draw(seed, (uint32_t)labels[i], t, DOM_FLIP, w);
+        spins[i] = store_of(q, mulhi_range(w[0], (uint32_t)q));
+    }
+}
+
+/* sat counts the 3N bonds; Ising E = -sum s_i s_j = -(2 sat - 3N), Potts E = -sat (Eq. 1) */
+void orc3_observables(int32_t L, int32_t q, const int8_t *spins, orc_obs *o)
+{
+    int64_t N = (int64_t)L * L * L;
+    memset(o, 0, sizeof(*o));
+    for (int64_t i = 0; i < N; ++i) {
+        int64_t nb[6];
+        nbrs3(L, i, nb);
+        for (int d = 0; d < 3; ++d) o->sat_bonds += (spins[i] == spins[nb[d]]);
+        int k = (q == 2) ? (spins[i] == 1 ? 0 : 1) : (int)(uint8_t)spins[i];
+        if (k >= 0 && k < 8) o->state_count[k] += 1;
+    }
+    if (q == 2) {
+        o->energy = -(2 * o->sat_bonds - 3 * N);
+        o->magnetisation = o->state_count[0] - o->state_count[1];
+    } else {
+        int64_t mx = 0;
+        for (int k = 0; k < q; ++k) if (o->state_count[k] > mx) mx = o->state_count[k];
+        o->energy = -o->sat_bonds;
+        o->magnetisation = (int64_t)q * mx - N;
+    }
+}
+
+int64_t orc3_sweep(int32_t L, int32_t q, uint32_t T, uint64_t seed, uint64_t t,
+                   int8_t *spins, int32_t *labels, uint8_t *codes, int64_t *active)
+{
+    int64_t N = (int64_t)L * L * L;
+    int own_labels = (labels == NULL), own_codes = (codes == NULL);
+    if (own_labels) labels = (int32_t *)malloc((size_t)N * sizeof(int32_t));
+    if (own_codes)  codes  = (uint8_t *)malloc((size_t)N);
+    if (!labels || !codes) return -1;
+    int64_t nb = orc3_bonds(L, T, seed, t, spins, codes);
+    int64_t nc = orc3_label(L, codes, labels);
+    orc3_flip(N, q, seed, t, labels, spins);
+    if (active) *active = nb;
+    if (own_labels) free(labels);
+    if (own_codes)  free(codes);
+    return nc;
+}
+
+/* series[4*s + 0..3] = energy, magnetisation, n_clusters, sum of squared cluster sizes */
+int orc3_run_chain(int32_t L, int32_t q, uint32_t T, uint64_t seed, uint64_t t0,
+                   int64_t n, int8_t *spins, int64_t *series)
+{
+    int64_t N = (int64_t)L * L * L;
+    int32_t *labels = (int32_t *)malloc((size_t)N * sizeof(int32_t));
+    uint8_t *codes = (uint8_t *)malloc((size_t)N);
+    if (!labels || !codes) return -1;
+    for (int64_t s = 0; s < n; ++s) {
+        int64_t nb = 0;
+        int64_t nc = orc3_sweep(L, q, T, seed, t0 + (uint64_t)s, spins, labels, codes, &nb);
+        if (series) {
+            orc_obs o; orc_cstats c;
+            orc3_observables(L, q, spins, &o);
+            orc_cluster_stats(N, labels, &c);
+            series[4 * s + 0] = o.energy;
+            series[4 * s + 1] = o.magnetisation;
+            series[4 * s + 2] = nc;
+            series[4 * s + 3] = (int64_t)c.sum_sq_cluster;
+        }
+    }
+    free(labels); free(codes);
+    return 0;
+}
