@@ -77,6 +77,18 @@ typedef struct {
 int sw_create(sw_handle** out, int32_t L, int32_t q, double beta, uint64_t seed);
 int sw_destroy(sw_handle* h);
 
+/* The same update on the periodic L x L x L SIMPLE CUBIC lattice (S:8f row 2; "hypercubic lattices": a site
+ * looks after "three out of six neighbours").  Site i = z L^2 + y L + x; it owns its bonds to the east (x+1), north (y+1)
+ * and up (z+1) neighbour; N = L^3.  Bond draws (reading 19): n(i,d) = [s_i == s_nbr(i,d)] and
+ * [PHILOX(seed; i, t, BOND3 = 4)[d] < T], d = 0 east, 1 north, 2 up -- one call per site.  Threshold, initialisation, flip
+ * and label convention are the square lattice's (the 2N of sw_obs / sw_series_read becomes 3N).  Requires 4 <= L <= 1024
+ * (N <= 2^30), L % 4 == 0, 2 <= q <= 8.  A cubic handle supports sw_bind (d_bonds: N bytes or NULL, workspace
+ * sw_workspace_bytes3d), sw_init_spins, sw_sweep, sw_sweep_host, sw_activate (one byte per site: bit 0 east, 1 north, 2 up),
+ * sw_observables(_ex), sw_cluster_stats, sw_series_read, the threshold / counter / profile calls; sw_label, wolff_step and
+ * sw_wolff_frontier return SW_EINVAL.  sw_profile_read phases: 0 = k3_local, 1 = k3_faces, 2 = k3_final. */
+int sw_create3d(sw_handle** out, int32_t L, int32_t q, double beta, uint64_t seed);
+size_t sw_workspace_bytes3d(int32_t L, int32_t q);
+
 /* Bytes of device workspace sw_bind needs for an L x L lattice (int32 strip-edge root arrays, int32 cluster-size scratch,
  * accumulators).  0 if L or q is invalid. */
 size_t sw_workspace_bytes(int32_t L, int32_t q);

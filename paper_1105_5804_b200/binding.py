@@ -21,7 +21,7 @@ SYMBOLS = [
     "sw_create", "sw_destroy", "sw_workspace_bytes", "sw_bind", "sw_set_threshold", "sw_get_threshold",
     "sw_set_counter", "sw_get_counter", "sw_init_spins", "sw_sweep", "sw_activate", "sw_label",
     "sw_cluster_stats", "wolff_step", "sw_observables", "sw_observables_ex", "sw_series_read", "sw_wolff_frontier", "sw_sweep_host", "sw_launch_count", "sw_strerror",
-    "sw_last_cuda_error", "sw_profile_enable", "sw_profile_read",
+    "sw_last_cuda_error", "sw_profile_enable", "sw_profile_read", "sw_create3d", "sw_workspace_bytes3d",
 ]
 
 
@@ -63,6 +63,9 @@ def lib():
     L.sw_destroy.argtypes = [vp]
     L.sw_workspace_bytes.argtypes = [i32, i32]
     L.sw_workspace_bytes.restype = C.c_size_t
+    L.sw_create3d.argtypes = [C.POINTER(vp), i32, i32, C.c_double, u64]
+    L.sw_workspace_bytes3d.argtypes = [i32, i32]
+    L.sw_workspace_bytes3d.restype = C.c_size_t
     L.sw_bind.argtypes = [vp, vp, vp, vp, vp, C.c_size_t, vp]
     L.sw_set_threshold.argtypes = [vp, u32]
     L.sw_get_threshold.argtypes = [vp, C.POINTER(u32)]
@@ -87,7 +90,7 @@ def lib():
     L.sw_last_cuda_error.argtypes = [vp]
     L.sw_last_cuda_error.restype = C.c_char_p
     for name in SYMBOLS:
-        if name not in ("sw_workspace_bytes", "sw_strerror", "sw_last_cuda_error"):
+        if name not in ("sw_workspace_bytes", "sw_workspace_bytes3d", "sw_strerror", "sw_last_cuda_error"):
             getattr(L, name).restype = C.c_int
     _lib = L
     return L
@@ -103,22 +106,26 @@ class SwError(RuntimeError):
 class Lattice:
     """One bound sw_handle plus the torch tensors it is bound to (device memory only; no arithmetic here)."""
 
-    def __init__(self, L: int, q: int, beta: float, seed: int, device="cuda:0", with_bonds: bool = False):
+    def __init__(self, L: int, q: int, beta: float, seed: int, device="cuda:0", with_bonds: bool = False, dim: int = 2):
+        """dim = 2: L x L square lattice (sw_create); dim = 3: L x L x L simple cubic lattice (sw_create3d)."""
         import torch
         self._torch = torch
         self._h = C.c_void_p()
         self._lib = lib()
-        rc = self._lib.sw_create(C.byref(self._h), L, q, beta, seed)
+        if dim not in (2, 3):
+            raise ValueError("dim must be 2 or 3")
+        rc = (self._lib.sw_create3d if dim == 3 else self._lib.sw_create)(C.byref(self._h), L, q, beta, seed)
         if rc != SW_OK:
             raise SwError(rc)
-        self.L, self.q, self.N = L, q, L * L
+        self.L, self.q, self.N, self.dim = L, q, L ** dim, dim
         self.device = torch.device(device)
         if self.device.type != "cuda":
             raise RuntimeError("swb200 needs a CUDA device; there is no CPU path")
         self.spins = torch.empty(self.N, dtype=torch.int8, device=self.device)
         self.labels = torch.empty(self.N, dtype=torch.int32, device=self.device)
-        self.bonds = torch.empty(self.N // 4, dtype=torch.uint8, device=self.device) if with_bonds else None
-        wb = self._lib.sw_workspace_bytes(L, q)
+        # bonds: packed, 4 sites per byte (square lattice); one byte per site (cubic lattice)
+        self.bonds = torch.empty(self.N // 4 if dim == 2 else self.N, dtype=torch.uint8, device=self.device) if with_bonds else None
+        wb = (self._lib.sw_workspace_bytes3d if dim == 3 else self._lib.sw_workspace_bytes)(L, q)
         self.work = torch.empty(wb, dtype=torch.uint8, device=self.device)
         self._check(self._lib.sw_bind(self._h, self.spins.data_ptr(), self.labels.data_ptr(),
                                       self.bonds.data_ptr() if with_bonds else None, self.work.data_ptr(), wb,

@@ -55,6 +55,8 @@ struct Params {
     uint32_t k1[10];     //                    k1[r] = seed_hi + r * 0xBB67AE85
     uint32_t negT;       // 2^32 - T (mod 2^32): u + negT carries iff u >= T, for T != 0 (scan_kernel.cuh shift_in_ge)
     uint32_t dmask;      // 0xFF; 0 if T = 0 (no bond is ever active)
+    int32_t  H;          // rows of the label array seen as H rows of L sites: L (square lattice) or L*L (simple cubic)
+    int32_t  n3x, n3y, n3z;   // simple cubic lattice: number of tiles per direction (cubic_kernels.cuh), else 0
 };
 
 // Philox4x32-10 (Salmon et al., SC'11).  c1,c2,c3 are warp-uniform in every use here (step counter and domain).

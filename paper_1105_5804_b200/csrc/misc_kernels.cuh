@@ -131,7 +131,7 @@ k_cluster_sizes(const Params p, const int* __restrict__ labels, int* __restrict_
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
     const int x = x0 + 4 * lane;
     if (x < L) {
-        for (int ly = warp; ly < TH && y0 + ly < L; ly += nwarp) {
+        for (int ly = warp; ly < TH && y0 + ly < p.H; ly += nwarp) {
             const int4 v = *reinterpret_cast<const int4*>(labels + (size_t)(y0 + ly) * L + x);
             int lab[4] = {v.x, v.y, v.z, v.w};
             int cnt[4] = {1, 1, 1, 1};

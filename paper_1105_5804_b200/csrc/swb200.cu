@@ -11,10 +11,12 @@
 #include "label_kernels.cuh"
 #include "misc_kernels.cuh"
 #include "wolff_kernel.cuh"
+#include "cubic_kernels.cuh"
 
 using namespace swb;
 
 struct sw_handle {
+    int32_t  dim;              // 2: L x L square lattice; 3: L x L x L simple cubic lattice (sw_create3d)
     int32_t  L, q;
     int64_t  N;
     double   beta;
@@ -27,6 +29,7 @@ struct sw_handle {
     int32_t*  d_labels;
     uint8_t*  d_bonds;
     uint8_t*  d_work;
+    uint8_t*  d_bonds3;            // simple cubic lattice: the bond bytes of the last sweep (N bytes of the workspace)
     // carved from d_work
     Acc*      d_acc;
     unsigned long long* d_wolff;   // WOLFF_RING slots
@@ -56,12 +59,13 @@ namespace {
 constexpr size_t ALIGN = 256;
 inline size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
-struct WorkLayout { size_t acc, wolff, wstatus, series, edgeA, edgeB, draws, size, total; };
+struct WorkLayout { size_t acc, wolff, wstatus, series, edgeA, edgeB, draws, size, bonds3, total; };
 
-WorkLayout work_layout(int32_t L)
+WorkLayout work_layout(int32_t L, int32_t dim)
 {
-    const size_t N = (size_t)L * L;
-    const size_t ntx = (L + TW - 1) / TW, nty = (L + TH - 1) / TH;
+    const size_t N = dim == 3 ? (size_t)L * L * L : (size_t)L * L;
+    // (the cubic path has no strips: no edge arrays, no draw cache; it keeps one bond byte per site)
+    const size_t ntx = dim == 3 ? 0 : (L + TW - 1) / TW, nty = dim == 3 ? 0 : (L + TH - 1) / TH;
     WorkLayout w;
     w.acc = 0;
     w.wolff = align_up(sizeof(Acc));
@@ -71,7 +75,8 @@ WorkLayout work_layout(int32_t L)
     w.edgeB = w.edgeA + align_up((ntx + nty) * (size_t)L * sizeof(int32_t));
     w.draws = w.edgeB + align_up((ntx + nty) * (size_t)L * sizeof(int32_t));
     w.size = w.draws + align_up(ntx * nty * (size_t)(TH / 4) * 32 * sizeof(uint32_t));
-    w.total = w.size + align_up(N * sizeof(int32_t));
+    w.bonds3 = w.size + align_up(N * sizeof(int32_t));
+    w.total = w.bonds3 + align_up(dim == 3 ? N : 0);
     return w;
 }
 
@@ -79,6 +84,11 @@ WorkLayout work_layout(int32_t L)
 bool valid_shape(int32_t L, int32_t q)
 {
     return L >= 4 && L <= 32768 && (L % 4) == 0 && q >= 2 && q <= 8 && (q == 2 || L <= 16384);
+}
+// simple cubic lattice: N = L^3 <= 2^30 (site indices and labels are int32)
+bool valid_shape3(int32_t L, int32_t q)
+{
+    return L >= 4 && L <= 1024 && (L % 4) == 0 && q >= 2 && q <= 8;
 }
 
 int cuda_fail(sw_handle* h, cudaError_t e, const char* where)
@@ -205,15 +215,16 @@ const char* sw_strerror(int code)
 
 const char* sw_last_cuda_error(const sw_handle* h) { return h ? h->cuda_err : ""; }
 
-int sw_create(sw_handle** out, int32_t L, int32_t q, double beta, uint64_t seed)
+static int create_any(sw_handle** out, int32_t dim, int32_t L, int32_t q, double beta, uint64_t seed)
 {
     if (!out) return SW_EINVAL;
     *out = nullptr;
-    if (!valid_shape(L, q) || !std::isfinite(beta) || beta < 0.0) return SW_EINVAL;
+    if (!(dim == 3 ? valid_shape3(L, q) : valid_shape(L, q)) || !std::isfinite(beta) || beta < 0.0) return SW_EINVAL;
     sw_handle* h = new (std::nothrow) sw_handle;
     if (!h) return SW_ENOMEM;
     memset(h, 0, sizeof(*h));
-    h->L = L; h->q = q; h->N = (int64_t)L * L; h->beta = beta; h->seed = seed; h->t = 0;
+    h->dim = dim;
+    h->L = L; h->q = q; h->N = dim == 3 ? (int64_t)L * L * L : (int64_t)L * L; h->beta = beta; h->seed = seed; h->t = 0;
     h->T = threshold_of(q, beta);
     Params& p = h->p;
     p.L = L; p.N = (int32_t)h->N; p.q = q;
@@ -221,6 +232,11 @@ int sw_create(sw_handle** out, int32_t L, int32_t q, double beta, uint64_t seed)
     p.sbit = h->N <= (1 << 28) ? 28 : 30;
     for (int k = 2; k <= 15; ++k) if ((1 << k) == L) p.logL = k;
     p.ntx = (L + TW - 1) / TW; p.nty = (L + TH - 1) / TH;
+    p.H = L;
+    if (dim == 3) {
+        p.H = L * L; p.nty = (p.H + TH - 1) / TH;        // (label array as L*L rows of L sites: cluster statistics)
+        p.n3x = (L + C3X - 1) / C3X; p.n3y = (L + C3Y - 1) / C3Y; p.n3z = (L + C3Z - 1) / C3Z;
+    }
     const uint32_t s_lo = (uint32_t)(seed & 0xFFFFFFFFu), s_hi = (uint32_t)(seed >> 32);
     for (int r = 0; r < 10; ++r) {
         p.k0[r] = s_lo + (uint32_t)r * 0x9E3779B9u;
@@ -229,6 +245,9 @@ int sw_create(sw_handle** out, int32_t L, int32_t q, double beta, uint64_t seed)
     *out = h;
     return SW_OK;
 }
+
+int sw_create(sw_handle** out, int32_t L, int32_t q, double beta, uint64_t seed) { return create_any(out, 2, L, q, beta, seed); }
+int sw_create3d(sw_handle** out, int32_t L, int32_t q, double beta, uint64_t seed) { return create_any(out, 3, L, q, beta, seed); }
 
 int sw_profile_enable(sw_handle* h, int on)
 {
@@ -275,7 +294,13 @@ int sw_destroy(sw_handle* h)
 size_t sw_workspace_bytes(int32_t L, int32_t q)
 {
     if (!valid_shape(L, q)) return 0;
-    return work_layout(L).total;
+    return work_layout(L, 2).total;
+}
+
+size_t sw_workspace_bytes3d(int32_t L, int32_t q)
+{
+    if (!valid_shape3(L, q)) return 0;
+    return work_layout(L, 3).total;
 }
 
 int sw_bind(sw_handle* h, void* d_spins, int32_t* d_labels, uint8_t* d_bonds, void* d_work, size_t work_bytes,
@@ -283,7 +308,7 @@ int sw_bind(sw_handle* h, void* d_spins, int32_t* d_labels, uint8_t* d_bonds, vo
 {
     if (!h || !d_spins || !d_labels || !d_work) return SW_EINVAL;
     if (((uintptr_t)d_spins | (uintptr_t)d_labels | (uintptr_t)d_bonds | (uintptr_t)d_work) & 15u) return SW_EINVAL;
-    const WorkLayout w = work_layout(h->L);
+    const WorkLayout w = work_layout(h->L, h->dim);
     if (work_bytes < w.total) return SW_EINVAL;
     h->d_spins = (uint32_t*)d_spins;
     h->d_labels = d_labels;
@@ -294,6 +319,7 @@ int sw_bind(sw_handle* h, void* d_spins, int32_t* d_labels, uint8_t* d_bonds, vo
     h->d_edgeA = (int32_t*)(h->d_work + w.edgeA);
     h->d_edgeB = (int32_t*)(h->d_work + w.edgeB);
     h->d_size = (int32_t*)(h->d_work + w.size);
+    h->d_bonds3 = h->d_work + w.bonds3;
     h->d_draws = (uint32_t*)(h->d_work + w.draws);
     h->d_series = (SeriesEntry*)(h->d_work + w.series);
     h->d_wolff_status = (int*)(h->d_work + w.wstatus);
@@ -322,11 +348,47 @@ int sw_init_spins(sw_handle* h, int mode, void* stream)
     return SW_OK;
 }
 
+// one sweep of the simple cubic lattice (cubic_kernels.cuh): k3_local -> k3_faces -> k3_final
+static int sweep3(sw_handle* h, cudaStream_t s)
+{
+    const Params p = params_at(h, h->t);
+    int rc = zero_sweep_counters(h, s);
+    if (rc) return rc;
+    const int ntiles = p.n3x * p.n3y * p.n3z;
+    const int gw = grid_capped(h->N / 4, 256, 148 * 16);
+    SW_PROF(h, 0, s);
+    if (h->q == 2) k3_local<true><<<ntiles, C3THREADS, 0, s>>>(p, h->d_spins, h->d_labels, h->d_bonds3, h->d_acc);
+    else           k3_local<false><<<ntiles, C3THREADS, 0, s>>>(p, h->d_spins, h->d_labels, h->d_bonds3, h->d_acc);
+    SW_LAUNCHED(h, "k3_local");
+    SW_PROF(h, 1, s);
+    k3_faces<<<gw, 256, 0, s>>>(p, h->d_bonds3, h->d_labels, h->d_acc, h->d_series);
+    SW_LAUNCHED(h, "k3_faces");
+    if (h->t != h->series_hi) h->series_lo = h->t;
+    h->series_hi = h->t + 1;
+    if (h->series_hi - h->series_lo > (uint64_t)SERIES_RING) h->series_lo = h->series_hi - SERIES_RING;
+    SW_PROF(h, 2, s);
+    if (h->q == 2) k3_final<true><<<gw, 256, 0, s>>>(p, h->d_labels, h->d_spins, h->d_acc);
+    else           k3_final<false><<<gw, 256, 0, s>>>(p, h->d_labels, h->d_spins, h->d_acc);
+    SW_LAUNCHED(h, "k3_final");
+    SW_PROF(h, 3, s);
+    if (h->prof_on && h->prof_n < PROF_MAX) ++h->prof_n;
+    ++h->t;
+    h->last_labels = h->d_labels;
+    return SW_OK;
+}
+
 int sw_sweep(sw_handle* h, int64_t n, void* stream)
 {
     if (!h || n < 0) return SW_EINVAL;
     if (!h->bound) return SW_ESTATE;
     cudaStream_t s = (cudaStream_t)stream;
+    if (h->dim == 3) {
+        for (int64_t k = 0; k < n; ++k) {
+            const int rc = sweep3(h, s);
+            if (rc) return rc;
+        }
+        return SW_OK;
+    }
     for (int64_t k = 0; k < n; ++k) {
         const Params p = params_at(h, h->t);
         int rc = zero_sweep_counters(h, s);
@@ -355,6 +417,13 @@ int sw_activate(sw_handle* h, void* stream)
     if (!h) return SW_EINVAL;
     if (!h->bound || !h->d_bonds) return SW_ESTATE;
     const Params p = params_at(h, h->t);
+    if (h->dim == 3) {                                   // one byte per site: bit 0 east, 1 north, 2 up
+        const int gw = grid_capped(h->N / 4, 256, 148 * 16);
+        if (h->q == 2) k3_activate<true><<<gw, 256, 0, (cudaStream_t)stream>>>(p, h->d_spins, h->d_bonds);
+        else           k3_activate<false><<<gw, 256, 0, (cudaStream_t)stream>>>(p, h->d_spins, h->d_bonds);
+        SW_LAUNCHED(h, "k3_activate");
+        return SW_OK;
+    }
     if (h->q == 2)
         k_activate<true><<<grid_capped(h->N / 16, 256, 148 * 16), 256, 0, (cudaStream_t)stream>>>(p, h->d_spins, h->d_bonds);
     else
@@ -365,7 +434,7 @@ int sw_activate(sw_handle* h, void* stream)
 
 int sw_label(sw_handle* h, const uint8_t* d_bonds_in, int32_t* d_labels_out, void* stream)
 {
-    if (!h) return SW_EINVAL;
+    if (!h || h->dim != 2) return SW_EINVAL;             // packed-bond labelling is defined for the square lattice only
     if (!h->bound) return SW_ESTATE;
     const uint8_t* bonds = d_bonds_in ? d_bonds_in : h->d_bonds;
     int32_t* labels = d_labels_out ? d_labels_out : h->d_labels;
@@ -443,7 +512,7 @@ static int wolff_step_labelling(sw_handle* h, unsigned long long* d_size_slot, b
 int wolff_step(sw_handle* h, int64_t n, int64_t* h_sizes, void* stream)
 {
     if (!h || n < 0) return SW_EINVAL;
-    if (h->q != 2) return SW_EINVAL;                     // DESIGN.md reading 8: the paper defines Wolff for Ising only
+    if (h->q != 2 || h->dim != 2) return SW_EINVAL;      // DESIGN.md reading 8: the paper defines Wolff for Ising only
     if (!h->bound) return SW_ESTATE;
     cudaStream_t s = (cudaStream_t)stream;
     const bool front = h->wolff_levels > 0;
@@ -503,7 +572,8 @@ int sw_observables_ex(sw_handle* h, sw_obs* h_out, int flags, void* stream)
     const Params p = params_at(h, h->t);
     if (flags & SW_OBS_SPINS) {
         SW_CUDA(h, cudaMemsetAsync(&h->d_acc->sat, 0, sizeof(unsigned long long) * 9, s));
-        k_observables<<<(h->L < 148 * 8 ? h->L : 148 * 8), 256, 0, s>>>(p, h->d_spins, h->d_acc);
+        if (h->dim == 3) k3_observables<<<grid_capped(h->N / 4, 256, 148 * 8), 256, 0, s>>>(p, h->d_spins, h->d_acc);
+        else             k_observables<<<(h->L < 148 * 8 ? h->L : 148 * 8), 256, 0, s>>>(p, h->d_spins, h->d_acc);
         SW_LAUNCHED(h, "k_observables");
     }
     const bool clusters = (flags & SW_OBS_CLUSTERS) && h->last_labels;
@@ -522,7 +592,7 @@ int sw_observables_ex(sw_handle* h, sw_obs* h_out, int flags, void* stream)
         for (int k = 1; k < h->q; ++k) { h_out->state_count[k] = (int64_t)a.cnt[k]; rest += (int64_t)a.cnt[k]; }
         h_out->state_count[0] = N - rest;
         if (h->q == 2) {
-            h_out->energy = -(2 * h_out->sat_bonds - 2 * N);
+            h_out->energy = -(2 * h_out->sat_bonds - (int64_t)h->dim * N);
             h_out->magnetisation = h_out->state_count[0] - h_out->state_count[1];
         } else {
             int64_t mx = 0;
@@ -569,7 +639,7 @@ int sw_series_read(sw_handle* h, uint64_t t_first, int64_t n, int64_t* h_energy,
     const int64_t N = h->N;
     for (int64_t k = 0; k < n; ++k) {
         const int64_t sat = (int64_t)buf[k].sat;
-        h_energy[k] = h->q == 2 ? -(2 * sat - 2 * N) : -sat;
+        h_energy[k] = h->q == 2 ? -(2 * sat - (int64_t)h->dim * N) : -sat;
         if (h_magnetisation) h_magnetisation[k] = N - 2 * (int64_t)buf[k].minus;
     }
     delete[] buf;
