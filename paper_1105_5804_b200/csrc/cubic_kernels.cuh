@@ -22,7 +22,16 @@
 
 namespace swb {
 
-constexpr int C3X = 32, C3Y = 8, C3Z = 8;                // tile: x extent = one 32-byte sector of spins, 128 bytes of labels
+#ifndef SWB_C3Y
+#define SWB_C3Y 8
+#endif
+#ifndef SWB_C3Z
+#define SWB_C3Z 8
+#endif
+#ifndef SWB_C3CTAS
+#define SWB_C3CTAS 8                                     // resident CTAs per SM k3_local is compiled for (32 registers): it is
+#endif                                                   // bound by shared-memory latency; 4 CTAs: 0.51 ms at L=256, 8: 0.36
+constexpr int C3X = 32, C3Y = SWB_C3Y, C3Z = SWB_C3Z;                // tile: x extent = one 32-byte sector of spins, 128 bytes of labels
 constexpr int C3SITES = C3X * C3Y * C3Z;
 constexpr int C3THREADS = 256;
 constexpr int C3ITEMS = C3SITES / 4 / C3THREADS;         // 32-bit spin words (4 sites) per thread
@@ -55,10 +64,18 @@ __device__ __forceinline__ uint32_t east_word(const uint32_t* __restrict__ spins
     return __funnelshift_r(w, spins_w[row + (xw + 1 == Lw ? 0 : xw + 1)], 8);
 }
 
-__device__ __forceinline__ int find_s(const volatile int* lab, int x)
+// find with path halving: a plain store of an ancestor into a non-root entry (roots change only by the atomicMin of
+// unite_s; a hook displaced by such a store is re-established by the retry loop there -- DESIGN.md "Concurrency")
+__device__ __forceinline__ int find_s(volatile int* lab, int x)
 {
     int pp = lab[x];
-    while (pp != x) { x = pp; pp = lab[x]; }
+    while (pp != x) {
+        const int gp = lab[pp];
+        if (gp == pp) return pp;
+        lab[x] = gp;
+        x = gp;
+        pp = lab[x];
+    }
     return x;
 }
 
@@ -89,7 +106,7 @@ __device__ __forceinline__ Tile3 tile3_of(const Params& p, int t)
 }
 
 template <bool ISING>
-__global__ void __launch_bounds__(C3THREADS, 4)
+__global__ void __launch_bounds__(C3THREADS, SWB_C3CTAS)
 k3_local(const Params p, const uint32_t* __restrict__ spins_w, int* __restrict__ prov, uint8_t* __restrict__ bonds,
          Acc* __restrict__ acc)
 {
@@ -120,26 +137,55 @@ k3_local(const Params p, const uint32_t* __restrict__ spins_w, int* __restrict__
             if (ISING) nminus += __popc(w & 0x80808080u);
         }
         s_bnd[l >> 2] = b;
-        *reinterpret_cast<int4*>(&s_lab[l]) = make_int4(l, l + 1, l + 2, l + 3);
+        // the runs along x inside the word are linked right away: a site points to the first site of its run
+        const int l1 = (b & 0x00000001u) ? l : l + 1, l2 = (b & 0x00000100u) ? l1 : l + 2, l3 = (b & 0x00010000u) ? l2 : l + 3;
+        *reinterpret_cast<int4*>(&s_lab[l]) = make_int4(l, l1, l2, l3);
     }
     __syncthreads();
-    // (2) unions over the bonds that stay inside the tile
+    // (2) unions over the bonds that stay inside the tile, one direction after the other: east links between words, then
+    // north, then (after pointing every site at its root, so that the finds of the last phase are one hop) up.  Interleaved,
+    // the up unions -- which join the largest sets -- cost 3x as much (0.36 -> see DESIGN.md).
 #pragma unroll
-    for (int k = 0; k < C3ITEMS; ++k) {
-        const int item = threadIdx.x + k * C3THREADS;
-        const int wx = item % (C3X / 4), r = item / (C3X / 4), ly = r % C3Y, lz = r / C3Y;
-        const int l = (lz * C3Y + ly) * C3X + 4 * wx;
-        const uint32_t b = s_bnd[l >> 2];
-        if (b == 0u) continue;
+    for (int dir = 0; dir < 3; ++dir) {
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const uint32_t bj = b >> (8 * j);
-            if ((bj & 1u) && 4 * wx + j + 1 < c.ex) unite_s(s_lab, l + j, l + j + 1);
-            if ((bj & 2u) && ly + 1 < c.ey) unite_s(s_lab, l + j, l + j + C3X);
-            if ((bj & 4u) && lz + 1 < c.ez) unite_s(s_lab, l + j, l + j + C3X * C3Y);
+        for (int k = 0; k < C3ITEMS; ++k) {
+            const int item = threadIdx.x + k * C3THREADS;
+            const int wx = item % (C3X / 4), r = item / (C3X / 4), ly = r % C3Y, lz = r / C3Y;
+            const int l = (lz * C3Y + ly) * C3X + 4 * wx;
+            const uint32_t b = s_bnd[l >> 2];
+            if (dir == 0) {
+                if ((b & 0x01000000u) && 4 * wx + 4 < c.ex) unite_s(s_lab, l + 3, l + 4);
+            } else if (dir == 1) {
+                if (ly + 1 < c.ey) {
+#pragma unroll
+                    for (int j = 0; j < 4; ++j)
+                        if (b & (2u << (8 * j))) unite_s(s_lab, l + j, l + j + C3X);
+                }
+            } else {
+                if (lz + 1 < c.ez) {
+#pragma unroll
+                    for (int j = 0; j < 4; ++j)
+                        if (b & (4u << (8 * j))) unite_s(s_lab, l + j, l + j + C3X * C3Y);
+                }
+            }
+        }
+        __syncthreads();
+        if (dir == 1) {
+#pragma unroll
+            for (int k = 0; k < C3ITEMS; ++k) {
+                const int item = threadIdx.x + k * C3THREADS;
+                const int wx = item % (C3X / 4), r = item / (C3X / 4), ly = r % C3Y, lz = r / C3Y;
+                const int l = (lz * C3Y + ly) * C3X + 4 * wx;
+                int rt[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) rt[j] = find_s(s_lab, l + j);
+                __syncthreads();                         // (all finds before any root's entry could be needed again: none is written)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) if (rt[j] != l + j) s_lab[l + j] = rt[j];
+            }
+            __syncthreads();
         }
     }
-    __syncthreads();
     // (3) every site -> the global index of its tile-local root
 #pragma unroll
     for (int k = 0; k < C3ITEMS; ++k) {
