@@ -252,21 +252,23 @@ k3_faces(const Params p, const uint8_t* __restrict__ bonds, int* prov, const Acc
         // which of the three bond directions of this word's sites leave their tile
         const bool facey = (y % C3Y) == C3Y - 1 || y == L - 1, facez = (z % C3Z) == C3Z - 1 || z == L - 1;
         const int i = 4 * i4;
+        if ((b & 0x01000000u) && (((x + 3) % C3X) == C3X - 1 || x + 3 == L - 1)) {        // east bond of the word's last site
+            const int nb = x + 3 == L - 1 ? i + 4 - L : i + 4;
+            gunite(prov, i + 3, nb, __ldcg(prov + i + 3), __ldcg(prov + nb));
+        }
+        // north / up bonds of the 4 sites: the entries of both sides are two 128-bit loads; a site whose two entries equal
+        // those of the previous site joins the same two trees (that site does the union)
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const uint32_t bj = b >> (8 * j);
-            const int xx = x + j;
-            if ((bj & 1u) && ((xx % C3X) == C3X - 1 || xx == L - 1)) {
-                const int nb = xx == L - 1 ? i + j + 1 - L : i + j + 1;
-                gunite(prov, i + j, nb, __ldcg(prov + i + j), __ldcg(prov + nb));
-            }
-            if ((bj & 2u) && facey) {
-                const int nb = y == L - 1 ? i + j - (L - 1) * L : i + j + L;
-                gunite(prov, i + j, nb, __ldcg(prov + i + j), __ldcg(prov + nb));
-            }
-            if ((bj & 4u) && facez) {
-                const int nb = z == L - 1 ? i + j - (L - 1) * L * L : i + j + L * L;
-                gunite(prov, i + j, nb, __ldcg(prov + i + j), __ldcg(prov + nb));
+        for (int d = 1; d < 3; ++d) {
+            if (!(d == 1 ? facey : facez) || !(b & (0x01010101u << d))) continue;
+            const int nb = d == 1 ? (y == L - 1 ? i - (L - 1) * L : i + L) : (z == L - 1 ? i - (L - 1) * L * L : i + L * L);
+            const int4 A4 = __ldcg(reinterpret_cast<const int4*>(prov + i)), B4 = __ldcg(reinterpret_cast<const int4*>(prov + nb));
+            const int A[4] = {A4.x, A4.y, A4.z, A4.w}, B[4] = {B4.x, B4.y, B4.z, B4.w};
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                if (!(b & ((1u << d) << (8 * j)))) continue;
+                if (j > 0 && (b & ((1u << d) << (8 * (j - 1)))) && A[j] == A[j - 1] && B[j] == B[j - 1]) continue;
+                gunite(prov, i + j, nb + j, A[j], B[j]);
             }
         }
     }
