@@ -35,6 +35,8 @@ COUNTERS_FILE = os.path.join(ROOT, "profiles", "r02_counters.json")
 EQUIL_SWEEPS = 100               # untimed sweeps before the timed region: SURVEY 8(d) "time sweeps 50-200", equilibrium state
 N_SMSP = 148 * 4
 BYTES_PER_SITE_LABEL = 12.25     # sw_label alone = packed bonds 0.25 + 4 + 4 + 4
+BYTES_PER_SITE_CUBIC = 15.0      # cubic_kernels.cuh: spin 1 + bond byte 1 + entry 4 | entry 4 + label 4 + spin 1
+BETA_C_CUBIC = 0.2216546         # critical coupling of the 3D Ising model (literature value; chooses the workload only)
 
 
 def kernel_source_hash() -> str:
@@ -314,6 +316,35 @@ def run_ours(args):
                                        "state": state_of(lb)}
             lb.close()
 
+    # ---- simple cubic lattice: a second workload, 3D Ising at its critical coupling ------------------
+    cubic = None
+    if rank == 0 and not args.no_cubic:
+        cubic = {}
+        for L3, nsw in ((256, 50), (512, 20)):
+            N3 = L3 ** 3
+            l3 = binding.Lattice(L3, 2, BETA_C_CUBIC, 1, device=device, dim=3)
+            l3.init_spins(1)
+            l3.sweep(60)
+            torch.cuda.synchronize()
+            ev0.record(stream)
+            l3.sweep(nsw)
+            ev1.record(stream)
+            torch.cuda.synchronize()
+            ms3 = ev0.elapsed_time(ev1) / nsw
+            l3.profile_enable(True); l3.sweep(nsw); ph3, n3 = l3.profile_read(); l3.profile_enable(False)
+            o3 = l3.observables()
+            gbs3 = BYTES_PER_SITE_CUBIC * N3 / (ms3 * 1e-3) / 1e9
+            cubic["L%d" % L3] = {"workload": "3D Ising (q=2) SW sweep, %d^3 periodic simple cubic lattice, beta=%.7f, 60 untimed + %d timed sweeps"
+                                             % (L3, BETA_C_CUBIC, nsw),
+                                 "ms_per_step": ms3, "ns_per_spin_update": ms3 * 1e6 / N3,
+                                 "algorithmic_bytes_per_site": BYTES_PER_SITE_CUBIC, "GB/s": gbs3,
+                                 "frac_of_measured_peak": gbs3 / measured_peak_gbs()[0],
+                                 "kernel_ms": {name: ph3[i] / max(1, n3) for i, name in enumerate(["k3_local", "k3_faces", "k3_final"])},
+                                 "state": {"energy_per_site": o3["energy"] / N3, "magnetisation_per_site": o3["magnetisation"] / N3,
+                                           "clusters_per_site": o3["n_clusters"] / N3,
+                                           "largest_cluster_fraction": o3["max_cluster"] / N3, "counter": o3["counter"]}}
+            l3.close()
+
     # ---- end to end through the host-buffer entry point ----------------------------------------------------
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
     h_in = torch.empty(N, dtype=torch.int8).pin_memory()
@@ -409,6 +440,7 @@ def run_ours(args):
         "cpu_baseline": cpu,
         "labelling": labelling,
         "other_betas": other_betas,
+        "cubic": cubic,
         "state_before_timed_region": state_before,
         "state": state_after,
     }
@@ -430,6 +462,7 @@ def main(argv=None):
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-labelling", action="store_true")
+    ap.add_argument("--no-cubic", action="store_true", help="skip the simple cubic lattice legs (SURVEY 8(f) row 2)")
     ap.add_argument("--no-other-betas", action="store_true", help="skip the beta = 0.40 / 0.50 legs of BASELINE.json configs[2]")
     ap.add_argument("--cpu-sweeps", type=int, default=3, help="oracle sweeps of the full lattice for cpu_baseline (0: L=4096 sample)")
     args = ap.parse_args(argv)

@@ -61,6 +61,15 @@ typedef struct {
     uint64_t counter;          /* step counter t after the last sweep / step                                  */
 } sw_obs;
 
+/* What the paper's own pipeline needed (sw_label_paper). */
+typedef struct {
+    int32_t selflabel_passes_max;   /* self-labelling passes of the slowest tile (n_B, Eq. 11)                   */
+    int32_t relax_iterations;       /* label-relaxation iterations until nothing changed (n_relax, Eq. 13); 0 for sewing */
+    int32_t sewing_levels;          /* levels of the hierarchical sewing (log2(L/B)); 0 for relaxation               */
+    int32_t reserved;
+    double  ms_local, ms_consolidate, ms_flatten;   /* CUDA-event times of the three phases                         */
+} sw_paper_stats;
+
 /* Cluster statistics of a canonical labelling (S:8a a9; BASELINE.json config 4 "cluster-size histogram"). */
 typedef struct {
     int64_t  n_clusters;
@@ -132,6 +141,16 @@ int sw_label(sw_handle* h, const uint8_t* d_bonds_in, int32_t* d_labels_out, voi
 
 /* Cluster statistics of canonical labels (d_labels_in == NULL: the bound d_labels).  Synchronises `stream`. */
 int sw_cluster_stats(sw_handle* h, const int32_t* d_labels_in, sw_cstats* h_out, void* stream);
+
+/* ABLATION BASELINE (S:8f row 4): the same labelling as sw_label, computed the way the PAPER does it -- self-labelling on
+ * B x B tiles in shared memory, then tile consolidation by label relaxation (method 0) or by
+ * hierarchical sewing (method 1), then a flatten pass -- so that the cost of the paper's design on a B200 can be put
+ * next to sw_label's.  Output: canonical labels (minimum site index), bit-identical to sw_label's.  B in {8, 16, 32}, L % B == 0,
+ * and L / B a power of two for method 1; square lattice only; else SW_EINVAL.  d_bonds_in / d_labels_out as in sw_label.
+ * Uses the cluster-size scratch of the workspace.  Synchronises `stream` (the relaxation's stopping criterion is read by the
+ * host between launches, as in the paper).  h_stats may be NULL.  Not on the sweep path. */
+int sw_label_paper(sw_handle* h, int method, int B, const uint8_t* d_bonds_in, int32_t* d_labels_out, sw_paper_stats* h_stats,
+                   void* stream);
 
 /* n Wolff single-cluster steps, q = 2 only (SW_EINVAL otherwise; reading 8); t += n.
  * Step at counter t (S:8c.9): seed site i0 = (PHILOX(seed; 0, t, WSEED)[0] * N) >> 32; C = component of i0 in the

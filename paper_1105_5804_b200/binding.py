@@ -21,7 +21,7 @@ SYMBOLS = [
     "sw_create", "sw_destroy", "sw_workspace_bytes", "sw_bind", "sw_set_threshold", "sw_get_threshold",
     "sw_set_counter", "sw_get_counter", "sw_init_spins", "sw_sweep", "sw_activate", "sw_label",
     "sw_cluster_stats", "wolff_step", "sw_observables", "sw_observables_ex", "sw_series_read", "sw_wolff_frontier", "sw_sweep_host", "sw_launch_count", "sw_strerror",
-    "sw_last_cuda_error", "sw_profile_enable", "sw_profile_read", "sw_create3d", "sw_workspace_bytes3d",
+    "sw_last_cuda_error", "sw_profile_enable", "sw_profile_read", "sw_create3d", "sw_workspace_bytes3d", "sw_label_paper",
 ]
 
 
@@ -44,6 +44,14 @@ class sw_cstats(C.Structure):
     def as_dict(self):
         return {"n_clusters": self.n_clusters, "max_cluster": self.max_cluster,
                 "sum_sq_cluster": self.sum_sq_cluster, "hist32": list(self.hist32)}
+
+
+class sw_paper_stats(C.Structure):
+    _fields_ = [("selflabel_passes_max", C.c_int32), ("relax_iterations", C.c_int32), ("sewing_levels", C.c_int32),
+                ("reserved", C.c_int32), ("ms_local", C.c_double), ("ms_consolidate", C.c_double), ("ms_flatten", C.c_double)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_ if k != "reserved"}
 
 
 _lib = None
@@ -76,6 +84,7 @@ def lib():
     L.sw_activate.argtypes = [vp, vp]
     L.sw_label.argtypes = [vp, vp, vp, vp]
     L.sw_cluster_stats.argtypes = [vp, vp, C.POINTER(sw_cstats), vp]
+    L.sw_label_paper.argtypes = [vp, C.c_int, C.c_int, vp, vp, C.POINTER(sw_paper_stats), vp]
     L.wolff_step.argtypes = [vp, i64, C.POINTER(i64), vp]
     L.sw_observables.argtypes = [vp, C.POINTER(sw_obs), vp]
     L.sw_observables_ex.argtypes = [vp, C.POINTER(sw_obs), C.c_int, vp]
@@ -180,6 +189,14 @@ class Lattice:
     def label(self, bonds=None, labels_out=None):
         self._check(self._lib.sw_label(self._h, bonds.data_ptr() if bonds is not None else None,
                                        labels_out.data_ptr() if labels_out is not None else None, self._stream()))
+
+    def label_paper(self, method: int, B: int, bonds=None, labels_out=None) -> dict:
+        """The paper's own pipeline (ablation baseline): method 0 = label relaxation, 1 = hierarchical sewing."""
+        st = sw_paper_stats()
+        self._check(self._lib.sw_label_paper(self._h, method, B, bonds.data_ptr() if bonds is not None else None,
+                                             labels_out.data_ptr() if labels_out is not None else None, C.byref(st),
+                                             self._stream()))
+        return st.as_dict()
 
     def cluster_stats(self, labels=None) -> dict:
         out = sw_cstats()

@@ -12,6 +12,7 @@
 #include "misc_kernels.cuh"
 #include "wolff_kernel.cuh"
 #include "cubic_kernels.cuh"
+#include "paper_kernels.cuh"
 
 using namespace swb;
 
@@ -561,6 +562,84 @@ int sw_wolff_frontier(sw_handle* h, int max_levels)
 {
     if (!h || max_levels < 0) return SW_EINVAL;
     h->wolff_levels = max_levels;
+    return SW_OK;
+}
+
+// The paper's own pipeline as an ablation baseline (paper_kernels.cuh): self-labelling on B x B tiles, then label relaxation
+// (method 0) or hierarchical sewing (method 1), then a flatten pass.
+int sw_label_paper(sw_handle* h, int method, int B, const uint8_t* d_bonds_in, int32_t* d_labels_out, sw_paper_stats* h_stats,
+                   void* stream)
+{
+    if (!h || h->dim != 2 || (method != 0 && method != 1) || (B != 8 && B != 16 && B != 32)) return SW_EINVAL;
+    if (!h->bound) return SW_ESTATE;
+    const int L = h->L;
+    int nt = L / B;
+    if (L % B != 0 || (method == 1 && (nt & (nt - 1)) != 0)) return SW_EINVAL;       // sewing pairs tiles level by level
+    const uint8_t* bonds = d_bonds_in ? d_bonds_in : h->d_bonds;
+    int32_t* labels = d_labels_out ? d_labels_out : h->d_labels;
+    if (!bonds) return SW_ESTATE;
+    if (((uintptr_t)bonds | (uintptr_t)labels) & 15u) return SW_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    int* const d_flag = h->d_wolff_status + 1;           // [0] belongs to the frontier Wolff kernel; [1] changed, [2] passes
+    int* const d_rlab = h->d_size;
+    cudaEvent_t ev[4];
+    for (int k = 0; k < 4; ++k) SW_CUDA(h, cudaEventCreate(&ev[k]));
+    int rc = zero_sweep_counters(h, s);
+    if (rc) return rc;
+    SW_CUDA(h, cudaMemsetAsync(d_flag, 0, 2 * sizeof(int), s));
+    SW_CUDA(h, cudaEventRecord(ev[0], s));
+    const dim3 tiles(nt, nt);
+    if (B == 8)       kp_selflabel<8><<<tiles, 64, 0, s>>>(L, bonds, labels, d_rlab, d_flag + 1);
+    else if (B == 16) kp_selflabel<16><<<tiles, 256, 0, s>>>(L, bonds, labels, d_rlab, d_flag + 1);
+    else              kp_selflabel<32><<<tiles, 1024, 0, s>>>(L, bonds, labels, d_rlab, d_flag + 1);
+    SW_LAUNCHED(h, "kp_selflabel");
+    SW_CUDA(h, cudaEventRecord(ev[1], s));
+    int iterations = 0, levels = 0;
+    unsigned long long* const d_ncl = &h->d_acc->part[0].n_clusters;
+    const int gN = grid_capped(h->N, 256, 148 * 16);
+    if (method == 0) {
+        const int gb = grid_capped(2 * (int64_t)nt * L, 256, 148 * 16);
+        while (true) {                                   // the stopping criterion is read by the host between launches
+            SW_CUDA(h, cudaMemsetAsync(d_flag, 0, sizeof(int), s));
+            kp_relax<<<gb, 256, 0, s>>>(L, B, bonds, labels, d_rlab, d_flag);
+            SW_LAUNCHED(h, "kp_relax");
+            ++iterations;
+            int changed = 0;
+            SW_CUDA(h, cudaMemcpyAsync(&changed, d_flag, sizeof(int), cudaMemcpyDeviceToHost, s));
+            SW_CUDA(h, cudaStreamSynchronize(s));
+            if (!changed) break;
+        }
+        SW_CUDA(h, cudaEventRecord(ev[2], s));
+        kp_flatten_relax<<<gN, 256, 0, s>>>((int)h->N, labels, d_rlab, d_ncl);
+        SW_LAUNCHED(h, "kp_flatten_relax");
+    } else {
+        for (int Bk = B; 2 * Bk <= L; Bk *= 2) {
+            kp_sew<<<dim3(L / (2 * Bk), L / (2 * Bk)), 32, 0, s>>>(L, Bk, bonds, labels);
+            SW_LAUNCHED(h, "kp_sew");
+            ++levels;
+        }
+        kp_sew_wrap<<<1, 32, 0, s>>>(L, bonds, labels);
+        SW_LAUNCHED(h, "kp_sew_wrap");
+        SW_CUDA(h, cudaEventRecord(ev[2], s));
+        kp_flatten<<<gN, 256, 0, s>>>((int)h->N, labels, d_ncl);
+        SW_LAUNCHED(h, "kp_flatten");
+    }
+    SW_CUDA(h, cudaEventRecord(ev[3], s));
+    int passes = 0;
+    SW_CUDA(h, cudaMemcpyAsync(&passes, d_flag + 1, sizeof(int), cudaMemcpyDeviceToHost, s));
+    SW_CUDA(h, cudaStreamSynchronize(s));
+    if (h_stats) {
+        float t01 = 0.f, t12 = 0.f, t23 = 0.f;
+        SW_CUDA(h, cudaEventElapsedTime(&t01, ev[0], ev[1]));
+        SW_CUDA(h, cudaEventElapsedTime(&t12, ev[1], ev[2]));
+        SW_CUDA(h, cudaEventElapsedTime(&t23, ev[2], ev[3]));
+        h_stats->selflabel_passes_max = passes;
+        h_stats->relax_iterations = iterations;
+        h_stats->sewing_levels = levels;
+        h_stats->ms_local = t01; h_stats->ms_consolidate = t12; h_stats->ms_flatten = t23;
+    }
+    for (int k = 0; k < 4; ++k) cudaEventDestroy(ev[k]);
+    h->last_labels = labels;
     return SW_OK;
 }
 
