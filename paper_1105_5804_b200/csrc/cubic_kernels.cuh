@@ -143,8 +143,8 @@ k3_local(const Params p, const uint32_t* __restrict__ spins_w, int* __restrict__
     }
     __syncthreads();
     // (2) unions over the bonds that stay inside the tile, one direction after the other: east links between words, then
-    // north, then (after pointing every site at its root, so that the finds of the last phase are one hop) up.  Interleaved,
-    // the up unions -- which join the largest sets -- cost 3x as much (0.36 -> see DESIGN.md).
+    // north, then up, every site pointed at its root in between (the finds of the next phase are one hop, and equal parents
+    // mean "united already").  Interleaved per site, the up unions -- which join the largest sets -- cost 3x as much.
 #pragma unroll
     for (int dir = 0; dir < 3; ++dir) {
 #pragma unroll
@@ -155,22 +155,26 @@ k3_local(const Params p, const uint32_t* __restrict__ spins_w, int* __restrict__
             const uint32_t b = s_bnd[l >> 2];
             if (dir == 0) {
                 if ((b & 0x01000000u) && 4 * wx + 4 < c.ex) unite_s(s_lab, l + 3, l + 4);
-            } else if (dir == 1) {
-                if (ly + 1 < c.ey) {
-#pragma unroll
-                    for (int j = 0; j < 4; ++j)
-                        if (b & (2u << (8 * j))) unite_s(s_lab, l + j, l + j + C3X);
-                }
             } else {
-                if (lz + 1 < c.ez) {
+                // north / up bonds of the 4 sites: the parents of both sides are two 128-bit loads (after the flatten below
+                // they are the roots so far); nothing to do where they are equal already, and a site whose two parents equal
+                // those of the previous bonded site joins the same two trees
+                const int off = dir == 1 ? C3X : C3X * C3Y;
+                const uint32_t m = (dir == 1 ? 0x02020202u : 0x04040404u) & b;
+                if (m != 0u && (dir == 1 ? ly + 1 < c.ey : lz + 1 < c.ez)) {
+                    const int4 A4 = *reinterpret_cast<const int4*>(&s_lab[l]), B4 = *reinterpret_cast<const int4*>(&s_lab[l + off]);
+                    const int A[4] = {A4.x, A4.y, A4.z, A4.w}, B[4] = {B4.x, B4.y, B4.z, B4.w};
 #pragma unroll
-                    for (int j = 0; j < 4; ++j)
-                        if (b & (4u << (8 * j))) unite_s(s_lab, l + j, l + j + C3X * C3Y);
+                    for (int j = 0; j < 4; ++j) {
+                        if (!(m & (0xFFu << (8 * j))) || A[j] == B[j]) continue;
+                        if (j > 0 && (m & (0xFFu << (8 * (j - 1)))) && A[j] == A[j - 1] && B[j] == B[j - 1]) continue;
+                        unite_s(s_lab, A[j], B[j]);
+                    }
                 }
             }
         }
         __syncthreads();
-        if (dir == 1) {
+        if (dir < 2) {
 #pragma unroll
             for (int k = 0; k < C3ITEMS; ++k) {
                 const int item = threadIdx.x + k * C3THREADS;
@@ -233,7 +237,14 @@ k3_activate(const Params p, const uint32_t* __restrict__ spins_w, uint8_t* __res
     }
 }
 
-// One thread per 4 sites.  series != NULL: one thread files the (sat, minus) totals of k3_local under the step counter.
+// Only the words that own bonds leaving their tile get a thread: ids [0, Wy) the words of the last row of every tile (north
+// bonds), [Wy, Wy + Wz) the words of the last plane of every tile (up bonds), then the last site of every tile row (east
+// bond).  series != NULL: one thread files the (sat, minus) totals of k3_local under the step counter.
+__host__ __device__ inline long long faces3_ids(int L)
+{
+    const long long Lw = L >> 2, nf = (L + C3Y - 1) / C3Y, nfz = (L + C3Z - 1) / C3Z, nfx = (L + C3X - 1) / C3X;
+    return (long long)L * nf * Lw + nfz * (long long)L * Lw + (long long)L * L * nfx;
+}
 __global__ void __launch_bounds__(256)
 k3_faces(const Params p, const uint8_t* __restrict__ bonds, int* prov, const Acc* __restrict__ acc,
          SeriesEntry* __restrict__ series)
@@ -244,33 +255,45 @@ k3_faces(const Params p, const uint8_t* __restrict__ bonds, int* prov, const Acc
         SeriesEntry e; e.sat = sat; e.minus = minus;
         series[p.t_lo & (SERIES_RING - 1)] = e;
     }
-    const int L = p.L, Lw = L >> 2, nw = p.N >> 2;
-    for (int i4 = blockIdx.x * blockDim.x + threadIdx.x; i4 < nw; i4 += gridDim.x * blockDim.x) {
-        const uint32_t b = reinterpret_cast<const uint32_t*>(bonds)[i4];
-        if (b == 0u) continue;
-        const int xw = i4 % Lw, r = i4 / Lw, y = r % L, z = r / L, x = 4 * xw;
-        // which of the three bond directions of this word's sites leave their tile
-        const bool facey = (y % C3Y) == C3Y - 1 || y == L - 1, facez = (z % C3Z) == C3Z - 1 || z == L - 1;
-        const int i = 4 * i4;
-        if ((b & 0x01000000u) && (((x + 3) % C3X) == C3X - 1 || x + 3 == L - 1)) {        // east bond of the word's last site
-            const int nb = x + 3 == L - 1 ? i + 4 - L : i + 4;
-            gunite(prov, i + 3, nb, __ldcg(prov + i + 3), __ldcg(prov + nb));
+    const int L = p.L, Lw = L >> 2;
+    const int nfy = (L + C3Y - 1) / C3Y, nfz = (L + C3Z - 1) / C3Z, nfx = (L + C3X - 1) / C3X;
+    const long long Wy = (long long)L * nfy * Lw, Wz = (long long)nfz * L * Lw;
+    long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (id < Wy + Wz) {
+        const int d = id < Wy ? 1 : 2;
+        int xw, y, z;
+        if (d == 1) {
+            xw = (int)(id % Lw); const long long r = id / Lw; const int fy = (int)(r % nfy); z = (int)(r / nfy);
+            y = min(fy * C3Y + C3Y - 1, L - 1);
+        } else {
+            id -= Wy;
+            xw = (int)(id % Lw); const long long r = id / Lw; y = (int)(r % L); const int fz = (int)(r / L);
+            z = min(fz * C3Z + C3Z - 1, L - 1);
         }
-        // north / up bonds of the 4 sites: the entries of both sides are two 128-bit loads; a site whose two entries equal
-        // those of the previous site joins the same two trees (that site does the union)
+        const int i = ((z * L + y) * Lw + xw) * 4;
+        const uint32_t b = reinterpret_cast<const uint32_t*>(bonds)[i >> 2] & (0x01010101u << d);
+        if (b == 0u) return;
+        const int nb = d == 1 ? (y == L - 1 ? i - (L - 1) * L : i + L) : (z == L - 1 ? i - (L - 1) * L * L : i + L * L);
+        // the entries of both sides are two 128-bit loads; a site whose two entries equal those of the previous bonded site
+        // joins the same two trees (that site does the union)
+        const int4 A4 = __ldcg(reinterpret_cast<const int4*>(prov + i)), B4 = __ldcg(reinterpret_cast<const int4*>(prov + nb));
+        const int A[4] = {A4.x, A4.y, A4.z, A4.w}, B[4] = {B4.x, B4.y, B4.z, B4.w};
 #pragma unroll
-        for (int d = 1; d < 3; ++d) {
-            if (!(d == 1 ? facey : facez) || !(b & (0x01010101u << d))) continue;
-            const int nb = d == 1 ? (y == L - 1 ? i - (L - 1) * L : i + L) : (z == L - 1 ? i - (L - 1) * L * L : i + L * L);
-            const int4 A4 = __ldcg(reinterpret_cast<const int4*>(prov + i)), B4 = __ldcg(reinterpret_cast<const int4*>(prov + nb));
-            const int A[4] = {A4.x, A4.y, A4.z, A4.w}, B[4] = {B4.x, B4.y, B4.z, B4.w};
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                if (!(b & ((1u << d) << (8 * j)))) continue;
-                if (j > 0 && (b & ((1u << d) << (8 * (j - 1)))) && A[j] == A[j - 1] && B[j] == B[j - 1]) continue;
-                gunite(prov, i + j, nb + j, A[j], B[j]);
-            }
+        for (int j = 0; j < 4; ++j) {
+            if (!(b & (0xFFu << (8 * j)))) continue;
+            if (j > 0 && (b & (0xFFu << (8 * (j - 1)))) && A[j] == A[j - 1] && B[j] == B[j - 1]) continue;
+            gunite(prov, i + j, nb + j, A[j], B[j]);
         }
+        return;
+    }
+    id -= Wy + Wz;
+    if (id < (long long)L * L * nfx) {
+        const int fx = (int)(id % nfx); const long long r = id / nfx;         // r = z L + y
+        const int x = min(fx * C3X + C3X - 1, L - 1);
+        const int i = (int)(r * L) + x;
+        if (!(bonds[i] & 1u)) return;
+        const int nb = x == L - 1 ? i + 1 - L : i + 1;
+        gunite(prov, i, nb, __ldcg(prov + i), __ldcg(prov + nb));
     }
 }
 

@@ -362,7 +362,7 @@ static int sweep3(sw_handle* h, cudaStream_t s)
     else           k3_local<false><<<ntiles, C3THREADS, 0, s>>>(p, h->d_spins, h->d_labels, h->d_bonds3, h->d_acc);
     SW_LAUNCHED(h, "k3_local");
     SW_PROF(h, 1, s);
-    k3_faces<<<gw, 256, 0, s>>>(p, h->d_bonds3, h->d_labels, h->d_acc, h->d_series);
+    k3_faces<<<(unsigned)((faces3_ids(h->L) + 255) / 256), 256, 0, s>>>(p, h->d_bonds3, h->d_labels, h->d_acc, h->d_series);
     SW_LAUNCHED(h, "k3_faces");
     if (h->t != h->series_hi) h->series_lo = h->t;
     h->series_hi = h->t + 1;
