@@ -307,15 +307,19 @@ k3_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __res
     for (int i4 = blockIdx.x * blockDim.x + threadIdx.x; i4 < nw; i4 += gridDim.x * blockDim.x) {
         const int4 v = *reinterpret_cast<const int4*>(labels + 4 * (size_t)i4);
         int rt[4] = {v.x, v.y, v.z, v.w};
+        // the four chases in lockstep: four independent loads per round trip (an entry is a parent pointer or, once its
+        // thread has been here, the final label: a root of the same tree either way)
+        int pp[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) pp[j] = __ldca(labels + rt[j]);
+        while ((pp[0] ^ rt[0]) | (pp[1] ^ rt[1]) | (pp[2] ^ rt[2]) | (pp[3] ^ rt[3])) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) { rt[j] = pp[j]; pp[j] = __ldca(labels + rt[j]); }
+        }
         uint32_t word = 0, state = 0;
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            if (j > 0 && rt[j] == (j == 1 ? v.x : j == 2 ? v.y : v.z)) {      // same tile-local root as the previous site
-                rt[j] = rt[j - 1];
-            } else {
-                rt[j] = gfind_cached(labels, rt[j]);
-                state = flip_state(p, rt[j]);
-            }
+            if (j == 0 || rt[j] != rt[j - 1]) state = flip_state(p, rt[j]);
             nroots += rt[j] == 4 * i4 + j;
             word |= (ISING ? (state ? 0xFFu : 0x01u) : state) << (8 * j);
         }
