@@ -189,6 +189,88 @@ def run_reference(args):
     return 0
 
 
+# ------------------------------------------------------------------------------------------------ ablation (S:8f row 4)
+def run_ablation(args):
+    """python bench.py --ablation: the paper's own labelling pipeline (sw_label_paper: self-labelling + relaxation / sewing) next
+    to sw_label on the bond sets of equilibrated critical configurations, L = 1024 .. --L.  One JSON line; not a bench line."""
+    import torch
+    from paper_1105_5804_b200 import binding
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU path")
+    rows = []
+    L = 1024
+    while L <= args.L:
+        lat = binding.Lattice(L, 2, args.beta, 1, with_bonds=True)
+        lat.init_spins(1)
+        lat.sweep(EQUIL_SWEEPS)
+        lat.activate()
+        ref = torch.empty(L * L, dtype=torch.int32, device="cuda")
+        lat.label(None, ref)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(5):
+            lat.label(None, ref)
+        e1.record()
+        torch.cuda.synchronize()
+        ours = e0.elapsed_time(e1) / 5
+        out = torch.empty(L * L, dtype=torch.int32, device="cuda")
+        for B in (8, 16, 32):
+            for method in (0, 1):
+                st = lat.label_paper(method, B, None, out)
+                rows.append({"L": L, "B": B, "consolidation": "relaxation" if method == 0 else "sewing",
+                             "labels_equal_sw_label": bool(torch.equal(out, ref)), "sw_label_ms": ours,
+                             "ms": st["ms_local"] + st["ms_consolidate"] + st["ms_flatten"], **st})
+        lat.close()
+        L *= 2
+    print(json.dumps({"ablation": "paper pipeline (P:152-258) vs sw_label, bonds of equilibrated configurations at beta=%.7f" % args.beta,
+                      "rows": rows}), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------ simple cubic lattice
+def cubic_leg(binding, torch, device, sizes):
+    """SW sweeps of the 3D Ising model at its critical coupling on L^3 periodic lattices: (L, timed sweeps) per entry."""
+    stream = torch.cuda.current_stream()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    cubic = {}
+    for L3, nsw in sizes:
+        N3 = L3 ** 3
+        l3 = binding.Lattice(L3, 2, BETA_C_CUBIC, 1, device=device, dim=3)
+        l3.init_spins(1)
+        l3.sweep(60)
+        torch.cuda.synchronize()
+        ev0.record(stream)
+        l3.sweep(nsw)
+        ev1.record(stream)
+        torch.cuda.synchronize()
+        ms3 = ev0.elapsed_time(ev1) / nsw
+        l3.profile_enable(True); l3.sweep(nsw); ph3, n3 = l3.profile_read(); l3.profile_enable(False)
+        o3 = l3.observables()
+        gbs3 = BYTES_PER_SITE_CUBIC * N3 / (ms3 * 1e-3) / 1e9
+        cubic["L%d" % L3] = {"workload": "3D Ising (q=2) SW sweep, %d^3 periodic simple cubic lattice, beta=%.7f, 60 untimed + %d timed sweeps"
+                                         % (L3, BETA_C_CUBIC, nsw),
+                             "ms_per_step": ms3, "ns_per_spin_update": ms3 * 1e6 / N3,
+                             "algorithmic_bytes_per_site": BYTES_PER_SITE_CUBIC, "GB/s": gbs3,
+                             "frac_of_measured_peak": gbs3 / measured_peak_gbs()[0],
+                             "kernel_ms": {name: ph3[i] / max(1, n3) for i, name in enumerate(["k3_local", "k3_faces", "k3_final"])},
+                             "state": {"energy_per_site": o3["energy"] / N3, "magnetisation_per_site": o3["magnetisation"] / N3,
+                                       "clusters_per_site": o3["n_clusters"] / N3,
+                                       "largest_cluster_fraction": o3["max_cluster"] / N3, "counter": o3["counter"]}}
+        l3.close()
+    return cubic
+
+
+def run_cubic_only(args):
+    """python bench.py --only-cubic: the simple cubic legs alone (used for the ncu capture of the k3_* kernels)."""
+    import torch
+    from paper_1105_5804_b200 import binding
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU path")
+    print(json.dumps({"cubic": cubic_leg(binding, torch, "cuda:0", ((256, 10),))}), flush=True)
+    return 0
+
+
 # ------------------------------------------------------------------------------------------------ our arm
 def run_ours(args):
     import torch
@@ -317,33 +399,7 @@ def run_ours(args):
             lb.close()
 
     # ---- simple cubic lattice: a second workload, 3D Ising at its critical coupling ------------------
-    cubic = None
-    if rank == 0 and not args.no_cubic:
-        cubic = {}
-        for L3, nsw in ((256, 50), (512, 20)):
-            N3 = L3 ** 3
-            l3 = binding.Lattice(L3, 2, BETA_C_CUBIC, 1, device=device, dim=3)
-            l3.init_spins(1)
-            l3.sweep(60)
-            torch.cuda.synchronize()
-            ev0.record(stream)
-            l3.sweep(nsw)
-            ev1.record(stream)
-            torch.cuda.synchronize()
-            ms3 = ev0.elapsed_time(ev1) / nsw
-            l3.profile_enable(True); l3.sweep(nsw); ph3, n3 = l3.profile_read(); l3.profile_enable(False)
-            o3 = l3.observables()
-            gbs3 = BYTES_PER_SITE_CUBIC * N3 / (ms3 * 1e-3) / 1e9
-            cubic["L%d" % L3] = {"workload": "3D Ising (q=2) SW sweep, %d^3 periodic simple cubic lattice, beta=%.7f, 60 untimed + %d timed sweeps"
-                                             % (L3, BETA_C_CUBIC, nsw),
-                                 "ms_per_step": ms3, "ns_per_spin_update": ms3 * 1e6 / N3,
-                                 "algorithmic_bytes_per_site": BYTES_PER_SITE_CUBIC, "GB/s": gbs3,
-                                 "frac_of_measured_peak": gbs3 / measured_peak_gbs()[0],
-                                 "kernel_ms": {name: ph3[i] / max(1, n3) for i, name in enumerate(["k3_local", "k3_faces", "k3_final"])},
-                                 "state": {"energy_per_site": o3["energy"] / N3, "magnetisation_per_site": o3["magnetisation"] / N3,
-                                           "clusters_per_site": o3["n_clusters"] / N3,
-                                           "largest_cluster_fraction": o3["max_cluster"] / N3, "counter": o3["counter"]}}
-            l3.close()
+    cubic = cubic_leg(binding, torch, device, ((256, 50), (512, 20))) if rank == 0 and not args.no_cubic else None
 
     # ---- end to end through the host-buffer entry point ----------------------------------------------------
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
@@ -462,6 +518,8 @@ def main(argv=None):
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-labelling", action="store_true")
+    ap.add_argument("--ablation", action="store_true", help="time the paper's own labelling pipeline next to sw_label (SURVEY 8(f) row 4)")
+    ap.add_argument("--only-cubic", action="store_true", help="run the L=256 simple cubic leg alone (ncu captures of the k3_* kernels)")
     ap.add_argument("--no-cubic", action="store_true", help="skip the simple cubic lattice legs (SURVEY 8(f) row 2)")
     ap.add_argument("--no-other-betas", action="store_true", help="skip the beta = 0.40 / 0.50 legs of BASELINE.json configs[2]")
     ap.add_argument("--cpu-sweeps", type=int, default=3, help="oracle sweeps of the full lattice for cpu_baseline (0: L=4096 sample)")
@@ -470,6 +528,10 @@ def main(argv=None):
         args.warmup = 3
     if args.impl == "reference":
         return run_reference(args)
+    if args.ablation:
+        return run_ablation(args)
+    if args.only_cubic:
+        return run_cubic_only(args)
     return run_ours(args)
 
 
