@@ -106,7 +106,10 @@ size_t sw_workspace_bytes(int32_t L, int32_t q);
  * d_bonds N/4 bytes of packed bonds or NULL (only sw_activate and sw_label(d_bonds=NULL) need it),
  * d_work >= sw_workspace_bytes(L,q) bytes.  Zeroes the accumulators in d_work on `stream`: later calls on this
  * handle must be ordered after that memset -- use the same stream, or synchronise `stream` before the first call on
- * another one.  (An argument the proposed signature of S:8b does not have; DESIGN.md section 1 lists the deviations.) */
+ * another one.  (An argument the proposed signature of S:8b does not have; DESIGN.md section 1 lists the deviations.)
+ * The CUDA device the buffers live on is read from d_spins (cudaPointerGetAttributes; SW_EINVAL if it is not device memory);
+ * every later call on the handle makes that device current for its own duration and restores the caller's, so a process
+ * with several GPUs need not cudaSetDevice around the library. */
 int sw_bind(sw_handle* h, void* d_spins, int32_t* d_labels, uint8_t* d_bonds, void* d_work, size_t work_bytes,
             void* stream);
 

@@ -46,6 +46,7 @@ struct sw_handle {
     uint64_t  draws_t;
     uint32_t  draws_T;
     bool      bound;
+    int       device;              // CUDA device the bound buffers live on (sw_bind); -1 before
     const int32_t* last_labels;    // labels buffer written by the LAST sweep / step / sw_label (NULL: none since bind)
     uint64_t  launches;
     char      cuda_err[256];
@@ -91,6 +92,19 @@ bool valid_shape3(int32_t L, int32_t q)
 {
     return L >= 4 && L <= 1024 && (L % 4) == 0 && q >= 2 && q <= 8;
 }
+
+// Every entry point that launches or copies makes the device of the bound buffers current for the call (a caller with
+// several GPUs need not have it current) and restores the previous one.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(const sw_handle* h)
+    {
+        if (h && h->device >= 0 && cudaGetDevice(&prev) == cudaSuccess && prev != h->device)
+            switched = cudaSetDevice(h->device) == cudaSuccess;
+    }
+    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
 
 int cuda_fail(sw_handle* h, cudaError_t e, const char* where)
 {
@@ -225,6 +239,7 @@ static int create_any(sw_handle** out, int32_t dim, int32_t L, int32_t q, double
     if (!h) return SW_ENOMEM;
     memset(h, 0, sizeof(*h));
     h->dim = dim;
+    h->device = -1;
     h->L = L; h->q = q; h->N = dim == 3 ? (int64_t)L * L * L : (int64_t)L * L; h->beta = beta; h->seed = seed; h->t = 0;
     h->T = threshold_of(q, beta);
     Params& p = h->p;
@@ -253,6 +268,7 @@ int sw_create3d(sw_handle** out, int32_t L, int32_t q, double beta, uint64_t see
 int sw_profile_enable(sw_handle* h, int on)
 {
     if (!h) return SW_EINVAL;
+    DeviceGuard guard(h);
     if (on && !h->prof_ev) {
         h->prof_ev = new (std::nothrow) cudaEvent_t[PROF_MAX * (SW_NPHASE + 1)];
         if (!h->prof_ev) return SW_ENOMEM;
@@ -267,6 +283,7 @@ int sw_profile_read(sw_handle* h, double ms[SW_NPHASE], uint64_t* n_sweeps)
 {
     if (!h || !ms || !n_sweeps) return SW_EINVAL;
     if (!h->prof_ev) return SW_ESTATE;
+    DeviceGuard guard(h);
     for (int k = 0; k < h->prof_n; ++k) {
         cudaEvent_t* e = h->prof_ev + k * (SW_NPHASE + 1);
         SW_CUDA(h, cudaEventSynchronize(e[SW_NPHASE]));
@@ -311,6 +328,15 @@ int sw_bind(sw_handle* h, void* d_spins, int32_t* d_labels, uint8_t* d_bonds, vo
     if (((uintptr_t)d_spins | (uintptr_t)d_labels | (uintptr_t)d_bonds | (uintptr_t)d_work) & 15u) return SW_EINVAL;
     const WorkLayout w = work_layout(h->L, h->dim);
     if (work_bytes < w.total) return SW_EINVAL;
+    {   // the device the buffers live on (a pointer that is not device memory is refused)
+        cudaPointerAttributes at;
+        if (cudaPointerGetAttributes(&at, d_spins) != cudaSuccess || (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged)) {
+            cudaGetLastError();
+            return SW_EINVAL;
+        }
+        h->device = at.device;
+    }
+    DeviceGuard guard(h);
     h->d_spins = (uint32_t*)d_spins;
     h->d_labels = d_labels;
     h->d_bonds = d_bonds;
@@ -343,6 +369,7 @@ int sw_init_spins(sw_handle* h, int mode, void* stream)
 {
     if (!h || (mode != 0 && mode != 1)) return SW_EINVAL;
     if (!h->bound) return SW_ESTATE;
+    DeviceGuard guard(h);
     const Params p = params_at(h, 0);
     k_init<<<grid_capped(h->N / 4, 256, 148 * 16), 256, 0, (cudaStream_t)stream>>>(p, h->d_spins, mode);
     SW_LAUNCHED(h, "k_init");
@@ -382,6 +409,7 @@ int sw_sweep(sw_handle* h, int64_t n, void* stream)
 {
     if (!h || n < 0) return SW_EINVAL;
     if (!h->bound) return SW_ESTATE;
+    DeviceGuard guard(h);
     cudaStream_t s = (cudaStream_t)stream;
     if (h->dim == 3) {
         for (int64_t k = 0; k < n; ++k) {
@@ -417,6 +445,7 @@ int sw_activate(sw_handle* h, void* stream)
 {
     if (!h) return SW_EINVAL;
     if (!h->bound || !h->d_bonds) return SW_ESTATE;
+    DeviceGuard guard(h);
     const Params p = params_at(h, h->t);
     if (h->dim == 3) {                                   // one byte per site: bit 0 east, 1 north, 2 up
         const int gw = grid_capped(h->N / 4, 256, 148 * 16);
@@ -437,6 +466,7 @@ int sw_label(sw_handle* h, const uint8_t* d_bonds_in, int32_t* d_labels_out, voi
 {
     if (!h || h->dim != 2) return SW_EINVAL;             // packed-bond labelling is defined for the square lattice only
     if (!h->bound) return SW_ESTATE;
+    DeviceGuard guard(h);
     const uint8_t* bonds = d_bonds_in ? d_bonds_in : h->d_bonds;
     int32_t* labels = d_labels_out ? d_labels_out : h->d_labels;
     if (!bonds) return SW_ESTATE;
@@ -474,6 +504,7 @@ int sw_cluster_stats(sw_handle* h, const int32_t* d_labels_in, sw_cstats* h_out,
 {
     if (!h || !h_out) return SW_EINVAL;
     if (!h->bound) return SW_ESTATE;
+    DeviceGuard guard(h);
     const int32_t* labels = d_labels_in ? d_labels_in : h->d_labels;
     if ((uintptr_t)labels & 15u) return SW_EINVAL;
     cudaStream_t s = (cudaStream_t)stream;
@@ -515,6 +546,7 @@ int wolff_step(sw_handle* h, int64_t n, int64_t* h_sizes, void* stream)
     if (!h || n < 0) return SW_EINVAL;
     if (h->q != 2 || h->dim != 2) return SW_EINVAL;      // DESIGN.md reading 8: the paper defines Wolff for Ising only
     if (!h->bound) return SW_ESTATE;
+    DeviceGuard guard(h);
     cudaStream_t s = (cudaStream_t)stream;
     const bool front = h->wolff_levels > 0;
     int64_t done = 0;
@@ -575,6 +607,7 @@ int sw_label_paper(sw_handle* h, int method, int B, const uint8_t* d_bonds_in, i
     const int L = h->L;
     int nt = L / B;
     if (L % B != 0 || (method == 1 && (nt & (nt - 1)) != 0)) return SW_EINVAL;       // sewing pairs tiles level by level
+    DeviceGuard guard(h);
     const uint8_t* bonds = d_bonds_in ? d_bonds_in : h->d_bonds;
     int32_t* labels = d_labels_out ? d_labels_out : h->d_labels;
     if (!bonds) return SW_ESTATE;
@@ -647,6 +680,7 @@ int sw_observables_ex(sw_handle* h, sw_obs* h_out, int flags, void* stream)
 {
     if (!h || !h_out || (flags & ~(SW_OBS_SPINS | SW_OBS_CLUSTERS))) return SW_EINVAL;
     if (!h->bound) return SW_ESTATE;
+    DeviceGuard guard(h);
     cudaStream_t s = (cudaStream_t)stream;
     const Params p = params_at(h, h->t);
     if (flags & SW_OBS_SPINS) {
@@ -703,6 +737,7 @@ int sw_series_read(sw_handle* h, uint64_t t_first, int64_t n, int64_t* h_energy,
 {
     if (!h || n < 0 || (n > 0 && !h_energy) || (h->q != 2 && h_magnetisation)) return SW_EINVAL;
     if (!h->bound) return SW_ESTATE;
+    DeviceGuard guard(h);
     if (n == 0) return SW_OK;
     if (t_first < h->series_lo || t_first + (uint64_t)n > h->series_hi) return SW_EINVAL;
     cudaStream_t s = (cudaStream_t)stream;
@@ -730,6 +765,7 @@ int sw_sweep_host(sw_handle* h, const void* h_spins_in, int64_t n, void* h_spins
 {
     if (!h || n < 0) return SW_EINVAL;
     if (!h->bound) return SW_ESTATE;
+    DeviceGuard guard(h);
     cudaStream_t s = (cudaStream_t)stream;
     if (h_spins_in) SW_CUDA(h, cudaMemcpyAsync(h->d_spins, h_spins_in, (size_t)h->N, cudaMemcpyHostToDevice, s));
     int rc = sw_sweep(h, n, stream);
