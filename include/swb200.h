@@ -93,8 +93,8 @@ int sw_destroy(sw_handle* h);
  * and label convention are the square lattice's (the 2N of sw_obs / sw_series_read becomes 3N).  Requires 4 <= L <= 1024
  * (N <= 2^30), L % 4 == 0, 2 <= q <= 8.  A cubic handle supports sw_bind (d_bonds: N bytes or NULL, workspace
  * sw_workspace_bytes3d), sw_init_spins, sw_sweep, sw_sweep_host, sw_activate (one byte per site: bit 0 east, 1 north, 2 up),
- * sw_observables(_ex), sw_cluster_stats, sw_series_read, the threshold / counter / profile calls; sw_label, wolff_step and
- * sw_wolff_frontier return SW_EINVAL.  sw_profile_read phases: 0 = k3_local, 1 = k3_faces, 2 = k3_final. */
+ * sw_label (bonds: one byte per site), sw_observables(_ex), sw_cluster_stats, sw_series_read, the threshold / counter / profile
+ * calls; wolff_step, sw_wolff_frontier and sw_label_paper return SW_EINVAL.  sw_profile_read phases: 0 = k3_local, 1 = k3_faces, 2 = k3_final. */
 int sw_create3d(sw_handle** out, int32_t L, int32_t q, double beta, uint64_t seed);
 size_t sw_workspace_bytes3d(int32_t L, int32_t q);
 

@@ -105,10 +105,12 @@ __device__ __forceinline__ Tile3 tile3_of(const Params& p, int t)
     return c;
 }
 
-template <bool ISING>
+// FROM_BONDS: the bond bytes are an INPUT (sw_label on a cubic handle: `bonds_in`, one byte per site); nothing is drawn,
+// no spins are read, no energy is counted.
+template <bool ISING, bool FROM_BONDS = false>
 __global__ void __launch_bounds__(C3THREADS, SWB_C3CTAS)
 k3_local(const Params p, const uint32_t* __restrict__ spins_w, int* __restrict__ prov, uint8_t* __restrict__ bonds,
-         Acc* __restrict__ acc)
+         Acc* __restrict__ acc, const uint8_t* __restrict__ bonds_in = nullptr)
 {
     __shared__ int s_lab[C3SITES];
     __shared__ uint32_t s_bnd[C3SITES / 4];
@@ -127,14 +129,18 @@ k3_local(const Params p, const uint32_t* __restrict__ spins_w, int* __restrict__
             const size_t row = ((size_t)z * L + y) * Lw;
             const size_t rown = ((size_t)z * L + (y + 1 == L ? 0 : y + 1)) * Lw;
             const size_t rowu = ((size_t)(z + 1 == L ? 0 : z + 1) * L + y) * Lw;
-            const uint32_t w = spins_w[row + xw];
-            uint32_t sat;
-            b = bonds3_word<ISING>(p, (uint32_t)((z * L + y) * L + x), w, east_word(spins_w, row, xw, Lw, w), spins_w[rown + xw],
-                                   spins_w[rowu + xw], sat);
+            if (FROM_BONDS) {
+                b = reinterpret_cast<const uint32_t*>(bonds_in)[row + xw] & 0x07070707u;
+            } else {
+                const uint32_t w = spins_w[row + xw];
+                uint32_t sat;
+                b = bonds3_word<ISING>(p, (uint32_t)((z * L + y) * L + x), w, east_word(spins_w, row, xw, Lw, w), spins_w[rown + xw],
+                                       spins_w[rowu + xw], sat);
+                nsat += sat;
+                if (ISING) nminus += __popc(w & 0x80808080u);
+            }
             reinterpret_cast<uint32_t*>(bonds)[row + xw] = b;
             nact += __popc(b);
-            nsat += sat;
-            if (ISING) nminus += __popc(w & 0x80808080u);
         }
         s_bnd[l >> 2] = b;
         // the runs along x inside the word are linked right away: a site points to the first site of its run
@@ -298,7 +304,8 @@ k3_faces(const Params p, const uint8_t* __restrict__ bonds, int* prov, const Acc
 }
 
 // One thread per 4 sites: canonical labels, new spins (flip == false: labels only), number of roots.
-template <bool ISING>
+// FLIP = false: labels only (sw_label)
+template <bool ISING, bool FLIP = true>
 __global__ void __launch_bounds__(256)
 k3_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __restrict__ acc)
 {
@@ -319,12 +326,12 @@ k3_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __res
         uint32_t word = 0, state = 0;
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            if (j == 0 || rt[j] != rt[j - 1]) state = flip_state(p, rt[j]);
+            if (FLIP && (j == 0 || rt[j] != rt[j - 1])) state = flip_state(p, rt[j]);
             nroots += rt[j] == 4 * i4 + j;
             word |= (ISING ? (state ? 0xFFu : 0x01u) : state) << (8 * j);
         }
         *reinterpret_cast<int4*>(labels + 4 * (size_t)i4) = make_int4(rt[0], rt[1], rt[2], rt[3]);
-        spins_w[i4] = word;
+        if (FLIP) spins_w[i4] = word;
     }
     nroots = __reduce_add_sync(FULLM, nroots);
     if ((threadIdx.x & 31) == 0 && nroots)

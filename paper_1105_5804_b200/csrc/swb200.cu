@@ -462,11 +462,34 @@ int sw_activate(sw_handle* h, void* stream)
     return SW_OK;
 }
 
+// sw_label on a cubic handle: one bond byte per site (bits 0-2) -> canonical labels
+static int label3(sw_handle* h, const uint8_t* bonds, int32_t* labels, cudaStream_t s)
+{
+    const Params p = params_at(h, h->t);
+    int rc = zero_sweep_counters(h, s);
+    if (rc) return rc;
+    k3_local<true, true><<<p.n3x * p.n3y * p.n3z, C3THREADS, 0, s>>>(p, nullptr, labels, h->d_bonds3, h->d_acc, bonds);
+    SW_LAUNCHED(h, "k3_local<bonds>");
+    k3_faces<<<(unsigned)((faces3_ids(h->L) + 255) / 256), 256, 0, s>>>(p, h->d_bonds3, labels, h->d_acc, nullptr);
+    SW_LAUNCHED(h, "k3_faces");
+    k3_final<true, false><<<grid_capped(h->N / 4, 256, 148 * 16), 256, 0, s>>>(p, labels, nullptr, h->d_acc);
+    SW_LAUNCHED(h, "k3_final<labels>");
+    h->last_labels = labels;
+    return SW_OK;
+}
+
 int sw_label(sw_handle* h, const uint8_t* d_bonds_in, int32_t* d_labels_out, void* stream)
 {
-    if (!h || h->dim != 2) return SW_EINVAL;             // packed-bond labelling is defined for the square lattice only
+    if (!h) return SW_EINVAL;
     if (!h->bound) return SW_ESTATE;
     DeviceGuard guard(h);
+    if (h->dim == 3) {
+        const uint8_t* b3 = d_bonds_in ? d_bonds_in : h->d_bonds;
+        int32_t* l3 = d_labels_out ? d_labels_out : h->d_labels;
+        if (!b3) return SW_ESTATE;
+        if (((uintptr_t)b3 | (uintptr_t)l3) & 15u) return SW_EINVAL;
+        return label3(h, b3, l3, (cudaStream_t)stream);
+    }
     const uint8_t* bonds = d_bonds_in ? d_bonds_in : h->d_bonds;
     int32_t* labels = d_labels_out ? d_labels_out : h->d_labels;
     if (!bonds) return SW_ESTATE;
@@ -592,7 +615,7 @@ int wolff_step(sw_handle* h, int64_t n, int64_t* h_sizes, void* stream)
 
 int sw_wolff_frontier(sw_handle* h, int max_levels)
 {
-    if (!h || max_levels < 0) return SW_EINVAL;
+    if (!h || max_levels < 0 || h->dim != 2) return SW_EINVAL;
     h->wolff_levels = max_levels;
     return SW_OK;
 }

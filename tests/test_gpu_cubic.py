@@ -97,6 +97,34 @@ def test_L128_equilibrated_from_gpu_state():
     lat.close()
 
 
+@pytest.mark.parametrize("L", [8, 20, 36, 64, 96])
+def test_label_bond_percolation_cubic(L):
+    """sw_label on a cubic handle: i.i.d. bond bytes (below, at and above the bond-percolation threshold 0.2488 of the simple
+    cubic lattice) and structured sets -> canonical labels, cluster count and statistics of the oracle."""
+    N = L ** 3
+    lat = binding.Lattice(L, 2, 0.1, 0, dim=3)
+    out = torch.empty(N, dtype=torch.int32, device="cuda")
+    rng = np.random.default_rng(L)
+    cases = []
+    for p in (0.15, 0.2488, 0.35):
+        c = np.zeros(N, dtype=np.uint8)
+        for d in range(3):
+            c |= (rng.random(N) < p).astype(np.uint8) << d
+        cases.append(c)
+    cases += [np.zeros(N, np.uint8), np.full(N, 7, np.uint8), np.full(N, 1, np.uint8), np.full(N, 2, np.uint8), np.full(N, 4, np.uint8)]
+    wrap = np.zeros(N, np.uint8)
+    wrap[L - 1] = 1; wrap[(L - 1) * L] |= 2; wrap[(L - 1) * L * L] |= 4            # one wrap bond per direction
+    cases.append(wrap)
+    for c in cases:
+        lat.label(torch.from_numpy(c).cuda(), out)
+        want, nc = oracle.label3(L, c)
+        got = out.cpu().numpy()
+        assert np.array_equal(got, want), f"L={L}: {int((got != want).sum())} labels differ"
+        assert lat.cluster_stats(out) == oracle.cluster_stats(want)
+        assert lat.observables(spins=False, clusters=False)["n_clusters"] == nc
+    lat.close()
+
+
 def test_unsupported_calls_and_shapes():
     lib = binding.lib()
     assert lib.sw_workspace_bytes3d(6, 2) == 0 and lib.sw_workspace_bytes3d(1028, 2) == 0 and lib.sw_workspace_bytes3d(64, 9) == 0
@@ -104,5 +132,6 @@ def test_unsupported_calls_and_shapes():
     with pytest.raises(binding.SwError):
         lat.wolff_step(1)
     with pytest.raises(binding.SwError):
-        lat.label()
+        lat.label_paper(0, 8)
+    assert lib.sw_wolff_frontier(lat._h, 8) == binding.SW_EINVAL
     lat.close()
