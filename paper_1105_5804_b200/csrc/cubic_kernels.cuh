@@ -148,53 +148,66 @@ k3_local(const Params p, const uint32_t* __restrict__ spins_w, int* __restrict__
         *reinterpret_cast<int4*>(&s_lab[l]) = make_int4(l, l1, l2, l3);
     }
     __syncthreads();
-    // (2) unions over the bonds that stay inside the tile, one direction after the other: east links between words, then
-    // north, then up, every site pointed at its root in between (the finds of the next phase are one hop, and equal parents
-    // mean "united already").  Interleaved per site, the up unions -- which join the largest sets -- cost 3x as much.
+    // (2) unions over the bonds that stay inside the tile.  East: the links between the words of a row, then every site is
+    // pointed at the root of its x-run.  North, then up: a thread WALKS a line of sites (north: fixed x and z, y = 0 .. C3Y-1,
+    // a warp per plane; up: fixed x and y, z = 0 .. C3Z-1, a warp per row) and carries the root of the set it is in: where the
+    // bond to the next site is active that site's tree is united with the carried root (one side of the union needs no
+    // find, and sets are joined bottom-up, so the trees stay shallow); where it is not, the walk continues with the next
+    // site's root.  Unions are lock-free (other lanes walk the neighbouring lines at the same time): atomicMin hook of the
+    // larger root under the smaller.  (One union per bond position of a word, direction by direction: 0.239 ms at L = 256;
+    // the walks: see DESIGN.md.)
+    static_assert(C3X == 32 && C3THREADS == C3X * C3Y && C3THREADS == C3X * C3Z, "one lane per x, one warp per plane / row");
 #pragma unroll
-    for (int dir = 0; dir < 3; ++dir) {
+    for (int k = 0; k < C3ITEMS; ++k) {
+        const int item = threadIdx.x + k * C3THREADS;
+        const int wx = item % (C3X / 4), r = item / (C3X / 4), ly = r % C3Y, lz = r / C3Y;
+        const int l = (lz * C3Y + ly) * C3X + 4 * wx;
+        if ((s_bnd[l >> 2] & 0x01000000u) && 4 * wx + 4 < c.ex) unite_s(s_lab, l + 3, l + 4);
+    }
+    __syncthreads();
+    {
+        int rt[C3ITEMS][4];
 #pragma unroll
         for (int k = 0; k < C3ITEMS; ++k) {
-            const int item = threadIdx.x + k * C3THREADS;
-            const int wx = item % (C3X / 4), r = item / (C3X / 4), ly = r % C3Y, lz = r / C3Y;
-            const int l = (lz * C3Y + ly) * C3X + 4 * wx;
-            const uint32_t b = s_bnd[l >> 2];
-            if (dir == 0) {
-                if ((b & 0x01000000u) && 4 * wx + 4 < c.ex) unite_s(s_lab, l + 3, l + 4);
-            } else {
-                // north / up bonds of the 4 sites: the parents of both sides are two 128-bit loads (after the flatten below
-                // they are the roots so far); nothing to do where they are equal already, and a site whose two parents equal
-                // those of the previous bonded site joins the same two trees
-                const int off = dir == 1 ? C3X : C3X * C3Y;
-                const uint32_t m = (dir == 1 ? 0x02020202u : 0x04040404u) & b;
-                if (m != 0u && (dir == 1 ? ly + 1 < c.ey : lz + 1 < c.ez)) {
-                    const int4 A4 = *reinterpret_cast<const int4*>(&s_lab[l]), B4 = *reinterpret_cast<const int4*>(&s_lab[l + off]);
-                    const int A[4] = {A4.x, A4.y, A4.z, A4.w}, B[4] = {B4.x, B4.y, B4.z, B4.w};
+            const int l = 4 * (threadIdx.x + k * C3THREADS);
 #pragma unroll
-                    for (int j = 0; j < 4; ++j) {
-                        if (!(m & (0xFFu << (8 * j))) || A[j] == B[j]) continue;
-                        if (j > 0 && (m & (0xFFu << (8 * (j - 1)))) && A[j] == A[j - 1] && B[j] == B[j - 1]) continue;
-                        unite_s(s_lab, A[j], B[j]);
-                    }
-                }
-            }
+            for (int j = 0; j < 4; ++j) rt[k][j] = find_s(s_lab, l + j);
         }
         __syncthreads();
-        if (dir < 2) {
 #pragma unroll
-            for (int k = 0; k < C3ITEMS; ++k) {
-                const int item = threadIdx.x + k * C3THREADS;
-                const int wx = item % (C3X / 4), r = item / (C3X / 4), ly = r % C3Y, lz = r / C3Y;
-                const int l = (lz * C3Y + ly) * C3X + 4 * wx;
-                int rt[4];
-#pragma unroll
-                for (int j = 0; j < 4; ++j) rt[j] = find_s(s_lab, l + j);
-                __syncthreads();                         // (all finds before any root's entry could be needed again: none is written)
-#pragma unroll
-                for (int j = 0; j < 4; ++j) if (rt[j] != l + j) s_lab[l + j] = rt[j];
-            }
-            __syncthreads();
+        for (int k = 0; k < C3ITEMS; ++k) {
+            const int l = 4 * (threadIdx.x + k * C3THREADS);
+            *reinterpret_cast<int4*>(&s_lab[l]) = make_int4(rt[k][0], rt[k][1], rt[k][2], rt[k][3]);
         }
+    }
+    __syncthreads();
+    const uint8_t* const s_bb = reinterpret_cast<const uint8_t*>(s_bnd);
+#pragma unroll
+    for (int dir = 1; dir < 3; ++dir) {
+        const int lx = threadIdx.x & (C3X - 1), other = threadIdx.x >> 5;        // north: other = z; up: other = y
+        const int stride = dir == 1 ? C3X : C3X * C3Y, n = dir == 1 ? c.ey : c.ez;
+        int l = (dir == 1 ? other * C3Y * C3X : other * C3X) + lx;
+        int root = s_lab[l];
+        for (int s = 0; s + 1 < n; ++s) {
+            const bool bond = (s_bb[l] >> dir) & 1u;
+            l += stride;
+            int a = root, b = s_lab[l];
+            root = b;
+            if (bond) {
+                while (true) {                           // unite; the carried root becomes the root of the union
+                    a = find_s(s_lab, a);
+                    b = find_s(s_lab, b);
+                    if (a == b) break;
+                    if (a < b) { const int t = a; a = b; b = t; }
+                    const int old = atomicMin(s_lab + a, b);
+                    if (old == a) { a = b; break; }
+                    a = old;
+                }
+                root = a;
+            }
+            __syncwarp();
+        }
+        __syncthreads();
     }
     // (3) every site -> the global index of its tile-local root
 #pragma unroll
