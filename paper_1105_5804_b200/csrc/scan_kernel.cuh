@@ -391,6 +391,9 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
     for (int i = threadIdx.x; i < 22; i += SCAN_THREADS)
         s_lb[i] = make_uint4(d_scan_lut.b[i][0], d_scan_lut.b[i][1], d_scan_lut.b[i][2], d_scan_lut.b[i][3]);
     __syncthreads();                                     // the only block-wide barrier
+#if SWB_PDL == 2
+    cudaGridDependencySynchronize();                     // (the tables do not depend on the preceding kernels)
+#endif
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int tx = blockIdx.x * SCAN_WARPS + warp, ty = blockIdx.y;

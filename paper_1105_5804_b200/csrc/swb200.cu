@@ -164,6 +164,21 @@ inline int prof_mark(sw_handle* h, int phase, cudaStream_t s)
 inline int grid_for(int64_t n, int block) { return (int)((n + block - 1) / block); }
 inline int grid_capped(int64_t n, int block, int cap) { int g = grid_for(n, block); return g < cap ? (g < 1 ? 1 : g) : cap; }
 
+#if SWB_PDL == 2
+// the per-sweep counters are zeroed by a kernel, so that the chain k_final -> k_zero -> k_scan is kernel to kernel
+__global__ void k_zero(Acc* acc)
+{
+    cudaGridDependencySynchronize();
+    reinterpret_cast<uint4*>(acc->part)[threadIdx.x] = make_uint4(0u, 0u, 0u, 0u);
+}
+inline cudaLaunchAttribute pdl_attr()
+{
+    cudaLaunchAttribute a;
+    a.id = cudaLaunchAttributeProgrammaticStreamSerialization; a.val.programmaticStreamSerializationAllowed = 1;
+    return a;
+}
+#endif
+
 // labelling of the bond graph of step t (or of packed bonds): k_scan -> k_seam; k_final resolves the rest
 // SRC_PHILOX falls through to SRC_DRAWS when the draw cache holds the draws of step t for the current threshold
 template <int SRC>
@@ -188,13 +203,36 @@ int launch_label_front(sw_handle* h, const Params& p, const uint8_t* bonds, int3
         SW_CUDA(h, cudaFuncSetAttribute((const void*)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(ScanSmem)));
         if (nopted < 16) opted[nopted++] = (const void*)kern;
     }
+#if SWB_PDL == 2
+    {
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = grid; cfg.blockDim = dim3(SCAN_THREADS); cfg.dynamicSmemBytes = sizeof(ScanSmem); cfg.stream = s;
+        cudaLaunchAttribute at[1] = {pdl_attr()};
+        cfg.attrs = at; cfg.numAttrs = 1;
+        SW_CUDA(h, cudaLaunchKernelEx(&cfg, kern, p, (const uint32_t*)h->d_spins, bonds, (const uint32_t*)h->d_draws, (int*)labels,
+                                      (int*)h->d_edgeA, (int*)h->d_edgeB, h->d_acc));
+    }
+#else
     kern<<<grid, SCAN_THREADS, sizeof(ScanSmem), s>>>(p, h->d_spins, bonds, h->d_draws, labels, h->d_edgeA, h->d_edgeB,
                                                       h->d_acc);
+#endif
     SW_LAUNCHED(h, "k_scan");
     SW_PROF(h, 1, s);
     const int nseam = (p.ntx + p.nty) * p.L;
+#if SWB_PDL
+    {
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(grid_for(seam_part(nseam), 256)); cfg.blockDim = dim3(256); cfg.stream = s;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        SW_CUDA(h, cudaLaunchKernelEx(&cfg, k_seam, p, (const int*)h->d_edgeA, (const int*)h->d_edgeB, (int*)labels,
+                                      (const Acc*)h->d_acc, record_series ? h->d_series : (SeriesEntry*)nullptr));
+    }
+#else
     k_seam<<<grid_for(seam_part(nseam), 256), 256, 0, s>>>(p, h->d_edgeA, h->d_edgeB, labels, h->d_acc,
                                                             record_series ? h->d_series : nullptr);
+#endif
     SW_LAUNCHED(h, "k_seam");
     if (record_series) {                                 // the ring now holds the entry of counter t
         if (t != h->series_hi) h->series_lo = t;
@@ -207,8 +245,18 @@ int launch_label_front(sw_handle* h, const Params& p, const uint8_t* bonds, int3
 
 int zero_sweep_counters(sw_handle* h, cudaStream_t s)
 {
+#if SWB_PDL == 2
+    static_assert(sizeof(AccPart) * ACC_PARTS == 256 * sizeof(uint4), "k_zero: one uint4 per thread");
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(1); cfg.blockDim = dim3(256); cfg.stream = s;
+    cudaLaunchAttribute at[1] = {pdl_attr()};
+    cfg.attrs = at; cfg.numAttrs = 1;
+    SW_CUDA(h, cudaLaunchKernelEx(&cfg, k_zero, h->d_acc));
+    ++h->launches;
+#else
     // the per-sweep counters (n_active, n_clusters) are the parts at the start of Acc
     SW_CUDA(h, cudaMemsetAsync(h->d_acc, 0, sizeof(AccPart) * ACC_PARTS, s));
+#endif
     return SW_OK;
 }
 
@@ -429,7 +477,17 @@ int sw_sweep(sw_handle* h, int64_t n, void* stream)
             const bool full = (p.L % TW) == 0 && (p.L % TH) == 0, q2 = p.q == 2;
             auto fin = full ? (q2 ? k_final<MODE_SW, GEN_ROWS, true, true> : k_final<MODE_SW, GEN_ROWS, true, false>)
                             : (q2 ? k_final<MODE_SW, GEN_ROWS, false, true> : k_final<MODE_SW, GEN_ROWS, false, false>);
+#if SWB_PDL
+            cudaLaunchConfig_t cfg = {};
+            cfg.gridDim = dim3(p.ntx, p.nty); cfg.blockDim = dim3(FIN_THREADS); cfg.stream = s;
+            cudaLaunchAttribute at[1];
+            at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[0].val.programmaticStreamSerializationAllowed = 1;
+            cfg.attrs = at; cfg.numAttrs = 1;
+            SW_CUDA(h, cudaLaunchKernelEx(&cfg, fin, p, (int*)h->d_labels, h->d_spins, h->d_acc, (unsigned long long*)nullptr,
+                                          h->d_draws));
+#else
             fin<<<dim3(p.ntx, p.nty), FIN_THREADS, 0, s>>>(p, h->d_labels, h->d_spins, h->d_acc, nullptr, h->d_draws);
+#endif
         }
         SW_LAUNCHED(h, "k_final<SW>");
         h->draws_valid = GEN_ROWS > 0; h->draws_t = h->t + 1; h->draws_T = h->T;
