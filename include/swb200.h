@@ -201,6 +201,29 @@ int sw_series_read(sw_handle* h, uint64_t t_first, int64_t n, int64_t* h_energy,
 int sw_sweep_host(sw_handle* h, const void* h_spins_in, int64_t n, void* h_spins_out, int32_t* h_labels_out,
                   sw_obs* h_obs, void* stream);
 
+/* MULTI-GPU ROW BANDS (S:8e, S:8f row 3; the paper proposes label relaxation between GPUs over MPI).  G processes, one
+ * GPU each, create the SAME lattice (same L, q, beta, seed, full-size buffers) and call sw_set_band(h, rank, G): the handle
+ * then works on the strip rows of band `rank` only (L % 32 == 0 and (L / 32) % G == 0; square lattice; SW_EINVAL otherwise;
+ * G = 1 restores the whole lattice).  One sweep of a banded handle:
+ *   1. the caller copies the spins of row y_halo (sw_band_layout) from the rank that owns it into the same row of d_spins;
+ *   2. sw_sweep_band_begin: activation + labelling of the band, seams inside the band, then the strip-local roots on the band's
+ *      two outer rows are replaced by the band's roots: L int32 rootN (last row; -1 where the north bond is inactive) at byte
+ *      offset work_off_rootN of d_work and L int32 rootS (first row) at work_off_rootS;
+ *   3. the caller all-gathers these two rows: the rows of band b of EVERY rank go to sw_band_layout(h, b, ...)'s offsets of
+ *      its own d_work (128 KiB per rank and sweep at L = 16384);
+ *   4. sw_sweep_band_end: every rank unites the G cross-band seams (redundantly, on its own full-size labels array), then
+ *      flattens and flips its band; t += 1.  d_labels / d_spins are valid in the band's rows [y_first, y_first + n_rows).
+ * The result is bit-identical to sw_sweep on one GPU (site indices, Philox counters and labels are global).  sw_band_counters
+ * returns this band's share of (active bonds, clusters, satisfied bonds and minus spins of the configuration the sweep
+ * started from): the caller sums them over the ranks.  sw_sweep, sw_label, wolff_step return SW_ESTATE on a banded handle.
+ * All asynchronous on `stream` except sw_band_counters, which synchronises. */
+int sw_set_band(sw_handle* h, int rank, int nranks);
+int sw_band_layout(const sw_handle* h, int band, int32_t* y_first, int32_t* n_rows, int32_t* y_halo,
+                   size_t* work_off_rootN, size_t* work_off_rootS);
+int sw_sweep_band_begin(sw_handle* h, void* stream);
+int sw_sweep_band_end(sw_handle* h, void* stream);
+int sw_band_counters(sw_handle* h, int64_t h_out[4], void* stream);
+
 /* Per-kernel timing of sw_sweep / sw_label with CUDA events on the launching stream (for roofline reporting; off by
  * default, and the un-instrumented path records no events).  While enabled, each sweep records SW_NPHASE+1
  * events; at most 512 sweeps are kept between reads (further sweeps run untimed).  sw_profile_read synchronises

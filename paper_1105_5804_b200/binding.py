@@ -22,6 +22,7 @@ SYMBOLS = [
     "sw_set_counter", "sw_get_counter", "sw_init_spins", "sw_sweep", "sw_activate", "sw_label",
     "sw_cluster_stats", "wolff_step", "sw_observables", "sw_observables_ex", "sw_series_read", "sw_wolff_frontier", "sw_sweep_host", "sw_launch_count", "sw_strerror",
     "sw_last_cuda_error", "sw_profile_enable", "sw_profile_read", "sw_create3d", "sw_workspace_bytes3d", "sw_label_paper",
+    "sw_set_band", "sw_band_layout", "sw_sweep_band_begin", "sw_sweep_band_end", "sw_band_counters",
 ]
 
 
@@ -85,6 +86,12 @@ def lib():
     L.sw_label.argtypes = [vp, vp, vp, vp]
     L.sw_cluster_stats.argtypes = [vp, vp, C.POINTER(sw_cstats), vp]
     L.sw_label_paper.argtypes = [vp, C.c_int, C.c_int, vp, vp, C.POINTER(sw_paper_stats), vp]
+    L.sw_set_band.argtypes = [vp, C.c_int, C.c_int]
+    L.sw_band_layout.argtypes = [vp, C.c_int, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), C.POINTER(C.c_size_t),
+                                 C.POINTER(C.c_size_t)]
+    L.sw_sweep_band_begin.argtypes = [vp, vp]
+    L.sw_sweep_band_end.argtypes = [vp, vp]
+    L.sw_band_counters.argtypes = [vp, C.POINTER(i64), vp]
     L.wolff_step.argtypes = [vp, i64, C.POINTER(i64), vp]
     L.sw_observables.argtypes = [vp, C.POINTER(sw_obs), vp]
     L.sw_observables_ex.argtypes = [vp, C.POINTER(sw_obs), C.c_int, vp]
@@ -197,6 +204,27 @@ class Lattice:
                                              labels_out.data_ptr() if labels_out is not None else None, C.byref(st),
                                              self._stream()))
         return st.as_dict()
+
+    # -- multi-GPU row bands (include/swb200.h "MULTI-GPU ROW BANDS"; the exchange itself is in bands.py) ----------------------
+    def set_band(self, rank: int, nranks: int):
+        self._check(self._lib.sw_set_band(self._h, rank, nranks))
+
+    def band_layout(self, band: int) -> dict:
+        y0, n, yh = C.c_int32(), C.c_int32(), C.c_int32()
+        oa, ob = C.c_size_t(), C.c_size_t()
+        self._check(self._lib.sw_band_layout(self._h, band, C.byref(y0), C.byref(n), C.byref(yh), C.byref(oa), C.byref(ob)))
+        return {"y_first": y0.value, "n_rows": n.value, "y_halo": yh.value, "off_rootN": oa.value, "off_rootS": ob.value}
+
+    def sweep_band_begin(self):
+        self._check(self._lib.sw_sweep_band_begin(self._h, self._stream()))
+
+    def sweep_band_end(self):
+        self._check(self._lib.sw_sweep_band_end(self._h, self._stream()))
+
+    def band_counters(self) -> dict:
+        out = (C.c_int64 * 4)()
+        self._check(self._lib.sw_band_counters(self._h, out, self._stream()))
+        return {"n_active_bonds": out[0], "n_clusters": out[1], "sat_before": out[2], "minus_before": out[3]}
 
     def cluster_stats(self, labels=None) -> dict:
         out = sw_cstats()

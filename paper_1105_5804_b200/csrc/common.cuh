@@ -57,6 +57,8 @@ struct Params {
     uint32_t dmask;      // 0xFF; 0 if T = 0 (no bond is ever active)
     int32_t  H;          // rows of the label array seen as H rows of L sites: L (square lattice) or L*L (simple cubic)
     int32_t  n3x, n3y, n3z;   // simple cubic lattice: number of tiles per direction (cubic_kernels.cuh), else 0
+    int32_t  ty0, nband;      // row band of a multi-GPU run (band_kernels.cuh): first strip row and number of strip rows this
+                              // handle works on; 0 and nty for the whole lattice
 };
 
 // Philox4x32-10 (Salmon et al., SC'11).  c1,c2,c3 are warp-uniform in every use here (step counter and domain).

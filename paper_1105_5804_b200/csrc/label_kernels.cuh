@@ -183,6 +183,9 @@ __host__ __device__ inline int seam_part(int nseam)     // ids per part, a multi
 
 // series != NULL (a sweep): one thread also files the (sat, minus) totals k_scan has just accumulated under the sweep's
 // counter, so that a chain keeps the energy and magnetisation of every configuration it passes through (sw_series_read).
+// BAND (multi-GPU row bands, band_kernels.cuh): only the seams INSIDE the band [ty0, ty0 + nband) of strip rows -- east seams of
+// its rows, north seams between its strip rows; the north seam on top of the band crosses to another rank.
+template <bool BAND>
 __global__ void __launch_bounds__(256)
 k_seam(const Params p, const int* __restrict__ edgeA, const int* __restrict__ edgeB, int* prov,
        const Acc* __restrict__ acc, SeriesEntry* __restrict__ series)
@@ -202,8 +205,15 @@ k_seam(const Params p, const int* __restrict__ edgeA, const int* __restrict__ ed
     int ra[SEAM_PER_THREAD], rb[SEAM_PER_THREAD], pa[SEAM_PER_THREAD], pb[SEAM_PER_THREAD];
     bool todo[SEAM_PER_THREAD];
 #pragma unroll
-    for (int k = 0; k < SEAM_PER_THREAD; ++k)
-        seam_ends(p, edgeA, edgeB, id < part ? id + k * part : nseam, nE, nseam, ra[k], rb[k]);
+    for (int k = 0; k < SEAM_PER_THREAD; ++k) {
+        int sid = id < part ? id + k * part : nseam;
+        if (BAND && sid < nseam) {
+            const int tr = sid < nE ? (sid - (int)div_L(p, (uint32_t)sid) * p.L) >> TH_LOG : (int)div_L(p, (uint32_t)(sid - nE));
+            const int hi = p.ty0 + p.nband - (sid < nE ? 0 : 1);
+            if (tr < p.ty0 || tr >= hi) sid = nseam;
+        }
+        seam_ends(p, edgeA, edgeB, sid, nE, nseam, ra[k], rb[k]);
+    }
 #pragma unroll
     for (int k = 0; k < SEAM_PER_THREAD; ++k) {
         todo[k] = seam_todo(ra[k], rb[k]);
@@ -285,7 +295,7 @@ k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __rest
     static_assert(R == 4, "flag words and draw words hold the 4 rows of a warp");
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int L = p.L;
-    const int x0 = blockIdx.x * TW, y0 = blockIdx.y * TH;
+    const int x0 = blockIdx.x * TW, y0 = (blockIdx.y + p.ty0) * TH;
     const int x = x0 + 4 * lane;
     const int ly0 = warp * R;
     const int base = y0 * L + x0;

@@ -396,7 +396,7 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
 #endif
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int tx = blockIdx.x * SCAN_WARPS + warp, ty = blockIdx.y;
+    const int tx = blockIdx.x * SCAN_WARPS + warp, ty = blockIdx.y + p.ty0;
     if (tx >= p.ntx) return;
     uint16_t* nm = sm.nm[warp];
     volatile uint16_t* vnm = nm;

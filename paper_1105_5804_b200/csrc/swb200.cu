@@ -13,6 +13,7 @@
 #include "wolff_kernel.cuh"
 #include "cubic_kernels.cuh"
 #include "paper_kernels.cuh"
+#include "band_kernels.cuh"
 
 using namespace swb;
 
@@ -47,6 +48,8 @@ struct sw_handle {
     uint32_t  draws_T;
     bool      bound;
     int       device;              // CUDA device the bound buffers live on (sw_bind); -1 before
+    int       band_rank, nbands;   // multi-GPU row bands (sw_set_band): this handle works on band band_rank of nbands; 0, 1 else
+    bool      band_open;           // sw_sweep_band_begin has run, sw_sweep_band_end has not
     const int32_t* last_labels;    // labels buffer written by the LAST sweep / step / sw_label (NULL: none since bind)
     uint64_t  launches;
     char      cuda_err[256];
@@ -186,7 +189,8 @@ int launch_label_front(sw_handle* h, const Params& p, const uint8_t* bonds, int3
                        bool record_series = false)
 {
     SW_PROF(h, 0, s);
-    const dim3 grid((p.ntx + SCAN_WARPS - 1) / SCAN_WARPS, p.nty);
+    const dim3 grid((p.ntx + SCAN_WARPS - 1) / SCAN_WARPS, p.nband);      // (nband = nty unless the handle works on a row band)
+    auto seam = h->nbands > 1 ? k_seam<true> : k_seam<false>;
     const bool ising = SRC == SRC_BONDS || p.q == 2, fullw = (p.L % TW) == 0;
     const uint64_t t = ((uint64_t)p.t_hi << 32) | p.t_lo;
     const bool cached = SRC == SRC_PHILOX && h->draws_valid && h->draws_t == t && h->draws_T == h->T;
@@ -226,12 +230,12 @@ int launch_label_front(sw_handle* h, const Params& p, const uint8_t* bonds, int3
         cudaLaunchAttribute at[1];
         at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[0].val.programmaticStreamSerializationAllowed = 1;
         cfg.attrs = at; cfg.numAttrs = 1;
-        SW_CUDA(h, cudaLaunchKernelEx(&cfg, k_seam, p, (const int*)h->d_edgeA, (const int*)h->d_edgeB, (int*)labels,
+        SW_CUDA(h, cudaLaunchKernelEx(&cfg, seam, p, (const int*)h->d_edgeA, (const int*)h->d_edgeB, (int*)labels,
                                       (const Acc*)h->d_acc, record_series ? h->d_series : (SeriesEntry*)nullptr));
     }
 #else
-    k_seam<<<grid_for(seam_part(nseam), 256), 256, 0, s>>>(p, h->d_edgeA, h->d_edgeB, labels, h->d_acc,
-                                                            record_series ? h->d_series : nullptr);
+    seam<<<grid_for(seam_part(nseam), 256), 256, 0, s>>>(p, h->d_edgeA, h->d_edgeB, labels, h->d_acc,
+                                                          record_series ? h->d_series : nullptr);
 #endif
     SW_LAUNCHED(h, "k_seam");
     if (record_series) {                                 // the ring now holds the entry of counter t
@@ -240,6 +244,26 @@ int launch_label_front(sw_handle* h, const Params& p, const uint8_t* bonds, int3
         if (h->series_hi - h->series_lo > (uint64_t)SERIES_RING) h->series_lo = h->series_hi - SERIES_RING;
     }
     SW_PROF(h, 2, s);
+    return SW_OK;
+}
+
+// flatten + flip of a sweep (k_final<MODE_SW>) over the strip rows the handle works on
+int launch_final_sw(sw_handle* h, const Params& p, cudaStream_t s)
+{
+    const bool full = (p.L % TW) == 0 && (p.L % TH) == 0, q2 = p.q == 2;
+    auto fin = full ? (q2 ? k_final<MODE_SW, GEN_ROWS, true, true> : k_final<MODE_SW, GEN_ROWS, true, false>)
+                    : (q2 ? k_final<MODE_SW, GEN_ROWS, false, true> : k_final<MODE_SW, GEN_ROWS, false, false>);
+#if SWB_PDL
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(p.ntx, p.nband); cfg.blockDim = dim3(FIN_THREADS); cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    SW_CUDA(h, cudaLaunchKernelEx(&cfg, fin, p, (int*)h->d_labels, h->d_spins, h->d_acc, (unsigned long long*)nullptr, h->d_draws));
+#else
+    fin<<<dim3(p.ntx, p.nband), FIN_THREADS, 0, s>>>(p, h->d_labels, h->d_spins, h->d_acc, nullptr, h->d_draws);
+#endif
+    SW_LAUNCHED(h, "k_final<SW>");
     return SW_OK;
 }
 
@@ -296,6 +320,8 @@ static int create_any(sw_handle** out, int32_t dim, int32_t L, int32_t q, double
     p.sbit = h->N <= (1 << 28) ? 28 : 30;
     for (int k = 2; k <= 15; ++k) if ((1 << k) == L) p.logL = k;
     p.ntx = (L + TW - 1) / TW; p.nty = (L + TH - 1) / TH;
+    p.ty0 = 0; p.nband = p.nty;
+    h->band_rank = 0; h->nbands = 1;
     p.H = L;
     if (dim == 3) {
         p.H = L * L; p.nty = (p.H + TH - 1) / TH;        // (label array as L*L rows of L sites: cluster statistics)
@@ -453,10 +479,91 @@ static int sweep3(sw_handle* h, cudaStream_t s)
     return SW_OK;
 }
 
+// ---- multi-GPU row bands (band_kernels.cuh) -----------------------------------------------------------------------------
+int sw_set_band(sw_handle* h, int rank, int nranks)
+{
+    if (!h || h->dim != 2 || nranks < 1 || rank < 0 || rank >= nranks) return SW_EINVAL;
+    if (h->p.nty % nranks != 0 || (h->L % TH) != 0) return SW_EINVAL;      // uniform bands of whole strip rows
+    h->band_rank = rank; h->nbands = nranks; h->band_open = false;
+    h->p.nband = h->p.nty / nranks;
+    h->p.ty0 = rank * h->p.nband;
+    return SW_OK;
+}
+
+int sw_band_layout(const sw_handle* h, int band, int32_t* y_first, int32_t* n_rows, int32_t* y_halo,
+                   size_t* work_off_rootN, size_t* work_off_rootS)
+{
+    if (!h || band < 0 || band >= h->nbands) return SW_EINVAL;
+    const int nb = h->p.nty / h->nbands, L = h->L;
+    const WorkLayout w = work_layout(h->L, h->dim);
+    const size_t nE = (size_t)h->p.ntx * L;
+    if (y_first) *y_first = band * nb * TH;
+    if (n_rows) *n_rows = nb * TH;
+    if (y_halo) *y_halo = ((band + 1) * nb * TH) % L;
+    if (work_off_rootN) *work_off_rootN = w.edgeA + (nE + (size_t)((band + 1) * nb - 1) * L) * sizeof(int32_t);
+    if (work_off_rootS) *work_off_rootS = w.edgeB + (nE + (size_t)(band * nb) * L) * sizeof(int32_t);
+    return SW_OK;
+}
+
+int sw_sweep_band_begin(sw_handle* h, void* stream)
+{
+    if (!h) return SW_EINVAL;
+    if (!h->bound || h->nbands < 2 || h->band_open) return SW_ESTATE;
+    DeviceGuard guard(h);
+    cudaStream_t s = (cudaStream_t)stream;
+    const Params p = params_at(h, h->t);
+    int rc = zero_sweep_counters(h, s);
+    if (rc) return rc;
+    rc = launch_label_front<SRC_PHILOX>(h, p, nullptr, h->d_labels, s, false);
+    if (rc) return rc;
+    k_band_resolve<<<grid_for(p.L, 256), 256, 0, s>>>(p, h->d_edgeA, h->d_edgeB, h->d_labels);
+    SW_LAUNCHED(h, "k_band_resolve");
+    h->band_open = true;
+    return SW_OK;
+}
+
+int sw_sweep_band_end(sw_handle* h, void* stream)
+{
+    if (!h) return SW_EINVAL;
+    if (!h->bound || h->nbands < 2 || !h->band_open) return SW_ESTATE;
+    DeviceGuard guard(h);
+    cudaStream_t s = (cudaStream_t)stream;
+    const Params p = params_at(h, h->t);
+    const int g = grid_for((int64_t)h->nbands * p.L, 256);
+    k_band_init<<<g, 256, 0, s>>>(p, h->d_edgeA, h->d_edgeB, h->d_labels, h->nbands);
+    SW_LAUNCHED(h, "k_band_init");
+    k_band_cross<<<g, 256, 0, s>>>(p, h->d_edgeA, h->d_edgeB, h->d_labels, h->nbands);
+    SW_LAUNCHED(h, "k_band_cross");
+    const int rc = launch_final_sw(h, p, s);
+    if (rc) return rc;
+    h->band_open = false;
+    h->series_lo = h->series_hi = h->t + 1;               // (the series counters cover a band only: not kept)
+    ++h->t;
+    h->last_labels = h->d_labels;
+    return SW_OK;
+}
+
+int sw_band_counters(sw_handle* h, int64_t h_out[4], void* stream)
+{
+    if (!h || !h_out) return SW_EINVAL;
+    if (!h->bound) return SW_ESTATE;
+    DeviceGuard guard(h);
+    cudaStream_t s = (cudaStream_t)stream;
+    Acc a;
+    SW_CUDA(h, cudaMemcpyAsync(&a, h->d_acc, sizeof(AccPart) * ACC_PARTS, cudaMemcpyDeviceToHost, s));
+    SW_CUDA(h, cudaStreamSynchronize(s));
+    h_out[0] = h_out[1] = h_out[2] = h_out[3] = 0;
+    for (int k = 0; k < ACC_PARTS; ++k) {
+        h_out[0] += (int64_t)a.part[k].n_active; h_out[1] += (int64_t)a.part[k].n_clusters;
+        h_out[2] += (int64_t)a.part[k].sat;      h_out[3] += (int64_t)a.part[k].minus;
+    }
+    return SW_OK;
+}
+
 int sw_sweep(sw_handle* h, int64_t n, void* stream)
 {
     if (!h || n < 0) return SW_EINVAL;
-    if (!h->bound) return SW_ESTATE;
+    if (!h->bound || h->nbands > 1) return SW_ESTATE;    // a banded handle sweeps through sw_sweep_band_begin / _end
     DeviceGuard guard(h);
     cudaStream_t s = (cudaStream_t)stream;
     if (h->dim == 3) {
@@ -472,24 +579,8 @@ int sw_sweep(sw_handle* h, int64_t n, void* stream)
         if (rc) return rc;
         rc = launch_label_front<SRC_PHILOX>(h, p, nullptr, h->d_labels, s, true);
         if (rc) return rc;
-        // the flatten + flip pass also draws the bonds of step t+1 (draw cache): the next sweep's k_scan only reads them
-        {
-            const bool full = (p.L % TW) == 0 && (p.L % TH) == 0, q2 = p.q == 2;
-            auto fin = full ? (q2 ? k_final<MODE_SW, GEN_ROWS, true, true> : k_final<MODE_SW, GEN_ROWS, true, false>)
-                            : (q2 ? k_final<MODE_SW, GEN_ROWS, false, true> : k_final<MODE_SW, GEN_ROWS, false, false>);
-#if SWB_PDL
-            cudaLaunchConfig_t cfg = {};
-            cfg.gridDim = dim3(p.ntx, p.nty); cfg.blockDim = dim3(FIN_THREADS); cfg.stream = s;
-            cudaLaunchAttribute at[1];
-            at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[0].val.programmaticStreamSerializationAllowed = 1;
-            cfg.attrs = at; cfg.numAttrs = 1;
-            SW_CUDA(h, cudaLaunchKernelEx(&cfg, fin, p, (int*)h->d_labels, h->d_spins, h->d_acc, (unsigned long long*)nullptr,
-                                          h->d_draws));
-#else
-            fin<<<dim3(p.ntx, p.nty), FIN_THREADS, 0, s>>>(p, h->d_labels, h->d_spins, h->d_acc, nullptr, h->d_draws);
-#endif
-        }
-        SW_LAUNCHED(h, "k_final<SW>");
+        rc = launch_final_sw(h, p, s);
+        if (rc) return rc;
         h->draws_valid = GEN_ROWS > 0; h->draws_t = h->t + 1; h->draws_T = h->T;
         SW_PROF(h, 3, s);
         if (h->prof_on && h->prof_n < PROF_MAX) ++h->prof_n;
@@ -541,6 +632,7 @@ int sw_label(sw_handle* h, const uint8_t* d_bonds_in, int32_t* d_labels_out, voi
     if (!h) return SW_EINVAL;
     if (!h->bound) return SW_ESTATE;
     DeviceGuard guard(h);
+    if (h->nbands > 1) return SW_ESTATE;
     if (h->dim == 3) {
         const uint8_t* b3 = d_bonds_in ? d_bonds_in : h->d_bonds;
         int32_t* l3 = d_labels_out ? d_labels_out : h->d_labels;
@@ -626,7 +718,7 @@ int wolff_step(sw_handle* h, int64_t n, int64_t* h_sizes, void* stream)
 {
     if (!h || n < 0) return SW_EINVAL;
     if (h->q != 2 || h->dim != 2) return SW_EINVAL;      // DESIGN.md reading 8: the paper defines Wolff for Ising only
-    if (!h->bound) return SW_ESTATE;
+    if (!h->bound || h->nbands > 1) return SW_ESTATE;
     DeviceGuard guard(h);
     cudaStream_t s = (cudaStream_t)stream;
     const bool front = h->wolff_levels > 0;
