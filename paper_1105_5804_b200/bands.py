@@ -101,10 +101,12 @@ class BandGroup:
 class DistBand:
     """One band per process; `dist` is an initialised torch.distributed (NCCL: one GPU per rank)."""
 
-    def __init__(self, L: int, q: int, beta: float, seed: int, dist, device):
+    def __init__(self, L: int, q: int, beta: float, seed: int, dist, device, lat=None):
+        """lat: an object with the band methods of binding.Lattice (the gloo test of the exchange passes a stand-in that holds
+        CPU tensors and launches nothing); default: a binding.Lattice on `device`."""
         self.dist, self.rank, self.G = dist, dist.get_rank(), dist.get_world_size()
         self.L, self.N = L, L * L
-        self.lat = binding.Lattice(L, q, beta, seed, device=device)
+        self.lat = lat if lat is not None else binding.Lattice(L, q, beta, seed, device=device)
         self.lat.set_band(self.rank, self.G)
         self.layout = [self.lat.band_layout(b) for b in range(self.G)]
 

@@ -285,7 +285,9 @@ __device__ __forceinline__ int fin_flag_site(int b)      // bit index -> r * TW 
 #else
 #define FIN_LD(p) __ldcs(p)
 #endif
-template <int MODE, int GENR, bool FULL, bool Q2>
+// BAND: the handle works on a row band (band_kernels.cuh): the strip row is blockIdx.y + ty0.  A template parameter, because
+// even this one addition in the whole-lattice kernels is measurable (k_final 0.5657 -> 0.5708 ms, k_scan 0.8637 -> 0.8656).
+template <int MODE, int GENR, bool FULL, bool Q2, bool BAND = false>
 __global__ void __launch_bounds__(FIN_THREADS, FIN_MIN_CTAS)
 k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __restrict__ acc,
         unsigned long long* __restrict__ wolff_size, uint32_t* __restrict__ draws)
@@ -295,7 +297,7 @@ k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __rest
     static_assert(R == 4, "flag words and draw words hold the 4 rows of a warp");
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int L = p.L;
-    const int x0 = blockIdx.x * TW, y0 = (blockIdx.y + p.ty0) * TH;
+    const int x0 = blockIdx.x * TW, y0 = (blockIdx.y + (BAND ? p.ty0 : 0)) * TH;
     const int x = x0 + 4 * lane;
     const int ly0 = warp * R;
     const int base = y0 * L + x0;

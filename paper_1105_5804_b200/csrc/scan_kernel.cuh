@@ -375,7 +375,7 @@ struct ScanSmem {
 // (`prov`, see label_kernels.cuh) and the edge arrays, and adds the number of active bonds to the sweep counters.
 // FULLW: L is a multiple of TW, every strip has all 32 lanes (no ragged right edge; the predicates fold away).
 enum { SRC_PHILOX = 0, SRC_BONDS = 1, SRC_DRAWS = 2 };
-template <int SRC, bool ISING, bool FULLW>
+template <int SRC, bool ISING, bool FULLW, bool BAND = false>    // BAND: strip row = blockIdx.y + ty0 (see k_final)
 __global__ void __launch_bounds__(SCAN_THREADS, 24 / SCAN_WARPS)    // 24 warps per SM (shared memory): up to 85 registers
 k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __restrict__ bonds_in,
        const uint32_t* __restrict__ draws, int* prov, int* __restrict__ edgeA, int* __restrict__ edgeB,
@@ -396,7 +396,7 @@ k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __re
 #endif
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int tx = blockIdx.x * SCAN_WARPS + warp, ty = blockIdx.y + p.ty0;
+    const int tx = blockIdx.x * SCAN_WARPS + warp, ty = blockIdx.y + (BAND ? p.ty0 : 0);
     if (tx >= p.ntx) return;
     uint16_t* nm = sm.nm[warp];
     volatile uint16_t* vnm = nm;

@@ -199,6 +199,9 @@ int launch_label_front(sw_handle* h, const Params& p, const uint8_t* bonds, int3
                                 : (fullw ? k_scan<SRC_DRAWS, false, true> : k_scan<SRC_DRAWS, false, false>))
                        : (ising ? (fullw ? k_scan<SRC_PHILOX, true, true> : k_scan<SRC_PHILOX, true, false>)
                                 : (fullw ? k_scan<SRC_PHILOX, false, true> : k_scan<SRC_PHILOX, false, false>));
+    if (h->nbands > 1)                                   // a row band: L is a multiple of TH, sweeps only (no draw cache)
+        kern = ising ? (fullw ? k_scan<SRC_PHILOX, true, true, true> : k_scan<SRC_PHILOX, true, false, true>)
+                     : (fullw ? k_scan<SRC_PHILOX, false, true, true> : k_scan<SRC_PHILOX, false, false, true>);
     static const void* opted[16];                        // kernels whose dynamic shared-memory limit has been raised
     static int nopted = 0;
     bool done = false;
@@ -253,6 +256,9 @@ int launch_final_sw(sw_handle* h, const Params& p, cudaStream_t s)
     const bool full = (p.L % TW) == 0 && (p.L % TH) == 0, q2 = p.q == 2;
     auto fin = full ? (q2 ? k_final<MODE_SW, GEN_ROWS, true, true> : k_final<MODE_SW, GEN_ROWS, true, false>)
                     : (q2 ? k_final<MODE_SW, GEN_ROWS, false, true> : k_final<MODE_SW, GEN_ROWS, false, false>);
+    if (h->nbands > 1)
+        fin = full ? (q2 ? k_final<MODE_SW, GEN_ROWS, true, true, true> : k_final<MODE_SW, GEN_ROWS, true, false, true>)
+                   : (q2 ? k_final<MODE_SW, GEN_ROWS, false, true, true> : k_final<MODE_SW, GEN_ROWS, false, false, true>);
 #if SWB_PDL
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(p.ntx, p.nband); cfg.blockDim = dim3(FIN_THREADS); cfg.stream = s;
