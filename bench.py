@@ -271,6 +271,83 @@ def run_cubic_only(args):
     return 0
 
 
+# ------------------------------------------------------------------------------------------------ row bands (S:8f row 3)
+def run_bands(args):
+    """python -m torch.distributed.run ... bench.py --gpus N --bands: ONE L x L lattice sharded into N row bands, one per GPU
+    (paper_1105_5804_b200/bands.py: a halo row of spins and two rows of roots are all-gathered per sweep).  Strong scaling:
+    the work is fixed, value = N sites / time.  Not the default (BASELINE.json: one GPU; `--gpus N` alone runs replicas)."""
+    import torch
+    import torch.distributed as dist
+    from paper_1105_5804_b200 import bands
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if world < 2:
+        raise SystemExit("--bands needs WORLD_SIZE >= 2 (torchrun); with one GPU run bench.py without it")
+    torch.cuda.set_device(local_rank)
+    dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    L, beta, N = args.L, args.beta, args.L * args.L
+    band = bands.DistBand(L, 2, beta, 1, dist, "cuda:%d" % local_rank)
+    band.init_spins(1)
+    band.sweep(max(EQUIL_SWEEPS, args.warmup))
+    stream = torch.cuda.current_stream()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    dist.barrier(); torch.cuda.synchronize()
+    ev0.record(stream)
+    band.sweep(args.steps)
+    ev1.record(stream)
+    dist.barrier(); torch.cuda.synchronize()
+    t = torch.tensor([ev0.elapsed_time(ev1)], dtype=torch.float64, device="cuda")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms = float(t.item())
+    c = band.counters()
+    if rank == 0:
+        ms = total_ms / args.steps
+        print(json.dumps({
+            "metric": "ns_per_spin_update", "value": ms * 1e6 / N, "unit": "ns", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": False, "scaling": "strong", "vs_baseline": None,
+            "dtype": "i32", "data": "synthetic",
+            "config": {"workload": "2D Ising (q=2) Swendsen-Wang, ONE L=%d periodic lattice in %d row bands, beta=%.10f" % (L, world, beta),
+                       "L": L, "q": 2, "beta": beta, "sites_per_step": N, "bands": world,
+                       "exchange_bytes_per_rank_and_sweep": L + 8 * L,
+                       "equilibration": "%d untimed sweeps" % max(EQUIL_SWEEPS, args.warmup)},
+            "state": {"clusters_per_site": c["n_clusters"] / N, "active_bonds_per_site": c["n_active_bonds"] / N,
+                      "energy_per_site_before_last_sweep": -(2 * c["sat_before"] - 2 * N) / N},
+            "frac_of_8TBps_nominal_per_gpu": BYTES_PER_SITE_SWEEP * N / world / (ms * 1e-3) / 1e9 / 8000.0}), flush=True)
+    band.close()
+    dist.destroy_process_group()
+    return 0
+
+
+def run_bands_one_gpu(args):
+    """python bench.py --bands-one-gpu G: the G-band algorithm run band after band on ONE GPU (bands.BandGroup): what the sharded
+    path costs in total GPU work next to sw_sweep (same lattice, same result) -- the per-band share is what one of G GPUs would
+    spend, link latency aside.  One JSON line; not a bench line."""
+    import torch
+    from paper_1105_5804_b200 import bands, binding
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU path")
+    L, beta, N, G = args.L, args.beta, args.L * args.L, args.bands_one_gpu
+    ref = binding.Lattice(L, 2, beta, 1)
+    ref.init_spins(1); ref.sweep(EQUIL_SWEEPS)
+    spins = ref.spins.clone(); t0 = ref.get_counter()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize(); ev0.record(); ref.sweep(args.steps); ev1.record(); torch.cuda.synchronize()
+    ms_ref = ev0.elapsed_time(ev1) / args.steps
+    grp = bands.BandGroup(L, 2, beta, 1, G)
+    for lat in grp.lats:                                  # the same equilibrated state on every band
+        lat.spins.copy_(spins); lat.set_counter(t0)
+    grp.sweep(3)
+    torch.cuda.synchronize(); ev0.record(); grp.sweep(args.steps - 3); ev1.record(); torch.cuda.synchronize()
+    ms_grp = ev0.elapsed_time(ev1) / max(1, args.steps - 3)
+    same = bool(torch.equal(torch.from_numpy(grp.spins_host()), ref.spins.cpu()))
+    print(json.dumps({"bands_one_gpu": G, "L": L, "beta": beta, "sw_sweep_ms": ms_ref, "all_bands_ms": ms_grp,
+                      "per_band_ms": ms_grp / G, "work_inflation": ms_grp / ms_ref,
+                      "spins_equal_single_gpu_chain_after_%d_sweeps" % args.steps: same}), flush=True)
+    grp.close(); ref.close()
+    return 0
+
+
 # ------------------------------------------------------------------------------------------------ our arm
 def run_ours(args):
     import torch
@@ -518,6 +595,8 @@ def main(argv=None):
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-labelling", action="store_true")
+    ap.add_argument("--bands", action="store_true", help="with --gpus N under torchrun: one lattice in N row bands (strong scaling) instead of N replicas")
+    ap.add_argument("--bands-one-gpu", type=int, default=0, metavar="G", help="time the G-band algorithm band after band on one GPU next to sw_sweep")
     ap.add_argument("--ablation", action="store_true", help="time the paper's own labelling pipeline next to sw_label (SURVEY 8(f) row 4)")
     ap.add_argument("--only-cubic", action="store_true", help="run the L=256 simple cubic leg alone (ncu captures of the k3_* kernels)")
     ap.add_argument("--no-cubic", action="store_true", help="skip the simple cubic lattice legs (SURVEY 8(f) row 2)")
@@ -532,6 +611,10 @@ def main(argv=None):
         return run_ablation(args)
     if args.only_cubic:
         return run_cubic_only(args)
+    if args.bands:
+        return run_bands(args)
+    if args.bands_one_gpu > 1:
+        return run_bands_one_gpu(args)
     return run_ours(args)
 
 

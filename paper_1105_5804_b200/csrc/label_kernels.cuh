@@ -181,6 +181,8 @@ __host__ __device__ inline int seam_part(int nseam)     // ids per part, a multi
     return ((nseam + 32 * SEAM_PER_THREAD - 1) / (32 * SEAM_PER_THREAD)) * 32;
 }
 
+__host__ __device__ inline int seam_band_sites(const Params& p) { return p.ntx * p.nband * TH + (p.nband - 1) * p.L; }
+
 // series != NULL (a sweep): one thread also files the (sat, minus) totals k_scan has just accumulated under the sweep's
 // counter, so that a chain keeps the energy and magnetisation of every configuration it passes through (sw_series_read).
 // BAND (multi-GPU row bands, band_kernels.cuh): only the seams INSIDE the band [ty0, ty0 + nband) of strip rows -- east seams of
@@ -200,17 +202,20 @@ k_seam(const Params p, const int* __restrict__ edgeA, const int* __restrict__ ed
         series[p.t_lo & (SERIES_RING - 1)] = e;
     }
     const int nE = p.ntx * p.L, nseam = (p.ntx + p.nty) * p.L;
-    const int part = seam_part(nseam);
+    // BAND: threads are enumerated over the band's own seam sites: ntx x (rows of the band) east sites, then the north sites
+    // of its strip rows but the last
+    const int bh = p.nband * TH, nlocal = BAND ? seam_band_sites(p) : nseam;
+    const int part = seam_part(nlocal);
     const int id = blockIdx.x * blockDim.x + threadIdx.x;
     int ra[SEAM_PER_THREAD], rb[SEAM_PER_THREAD], pa[SEAM_PER_THREAD], pb[SEAM_PER_THREAD];
     bool todo[SEAM_PER_THREAD];
 #pragma unroll
     for (int k = 0; k < SEAM_PER_THREAD; ++k) {
-        int sid = id < part ? id + k * part : nseam;
-        if (BAND && sid < nseam) {
-            const int tr = sid < nE ? (sid - (int)div_L(p, (uint32_t)sid) * p.L) >> TH_LOG : (int)div_L(p, (uint32_t)(sid - nE));
-            const int hi = p.ty0 + p.nband - (sid < nE ? 0 : 1);
-            if (tr < p.ty0 || tr >= hi) sid = nseam;
+        int sid = id < part ? id + k * part : nlocal;
+        if (BAND) {
+            if (sid >= nlocal) sid = nseam;
+            else if (sid < p.ntx * bh) { const int tc = sid / bh; sid = tc * p.L + p.ty0 * TH + (sid - tc * bh); }
+            else sid = nE + p.ty0 * p.L + (sid - p.ntx * bh);
         }
         seam_ends(p, edgeA, edgeB, sid, nE, nseam, ra[k], rb[k]);
     }

@@ -225,7 +225,7 @@ int launch_label_front(sw_handle* h, const Params& p, const uint8_t* bonds, int3
 #endif
     SW_LAUNCHED(h, "k_scan");
     SW_PROF(h, 1, s);
-    const int nseam = (p.ntx + p.nty) * p.L;
+    const int nseam = h->nbands > 1 ? seam_band_sites(p) : (p.ntx + p.nty) * p.L;
 #if SWB_PDL
     {
         cudaLaunchConfig_t cfg = {};
