@@ -215,7 +215,8 @@ int sw_sweep_host(sw_handle* h, const void* h_spins_in, int64_t n, void* h_spins
  *      flattens and flips its band; t += 1.  d_labels / d_spins are valid in the band's rows [y_first, y_first + n_rows).
  * The result is bit-identical to sw_sweep on one GPU (site indices, Philox counters and labels are global).  sw_band_counters
  * returns this band's share of (active bonds, clusters, satisfied bonds and minus spins of the configuration the sweep
- * started from): the caller sums them over the ranks.  sw_sweep, sw_label, wolff_step return SW_ESTATE on a banded handle.
+ * started from): the caller sums them over the ranks.  sw_sweep, sw_sweep_host, sw_label, sw_activate, wolff_step,
+ * sw_observables(_ex) and sw_cluster_stats on the bound labels return SW_ESTATE on a banded handle (it holds its band's rows only).
  * All asynchronous on `stream` except sw_band_counters, which synchronises. */
 int sw_set_band(sw_handle* h, int rank, int nranks);
 int sw_band_layout(const sw_handle* h, int band, int32_t* y_first, int32_t* n_rows, int32_t* y_halo,

@@ -94,6 +94,10 @@ def test_band_arguments_and_states():
     lat.set_band(1, 2)
     assert lib.sw_sweep(lat._h, 1, None) == binding.SW_ESTATE
     assert lib.sw_sweep_band_end(lat._h, None) == binding.SW_ESTATE     # begin has not run
+    with pytest.raises(binding.SwError):
+        lat.observables()                                            # a banded handle holds its band's rows only
+    with pytest.raises(binding.SwError):
+        lat.wolff_step(1)
     lay = lat.band_layout(1)
     assert lay["y_first"] == 128 and lay["n_rows"] == 128 and lay["y_halo"] == 0
     lat.set_band(0, 1)                                               # back to the whole lattice
