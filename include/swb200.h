@@ -200,6 +200,10 @@ int sw_series_read(sw_handle* h, uint64_t t_first, int64_t n, int64_t* h_energy,
  * NULL), fill h_obs (may be NULL).  Synchronises `stream`. */
 int sw_sweep_host(sw_handle* h, const void* h_spins_in, int64_t n, void* h_spins_out, int32_t* h_labels_out,
                   sw_obs* h_obs, void* stream);
+/* The same with the parts of h_obs chosen as in sw_observables_ex (SW_OBS_SPINS alone skips the cluster-size pass, 2 ms at
+ * L = 16384: energy, magnetisation, state counts, n_clusters and n_active_bonds are still filled). */
+int sw_sweep_host_ex(sw_handle* h, const void* h_spins_in, int64_t n, void* h_spins_out, int32_t* h_labels_out,
+                     sw_obs* h_obs, int obs_flags, void* stream);
 
 /* MULTI-GPU ROW BANDS (S:8e, S:8f row 3; the paper proposes label relaxation between GPUs over MPI).  G processes, one
  * GPU each, create the SAME lattice (same L, q, beta, seed, full-size buffers) and call sw_set_band(h, rank, G): the handle

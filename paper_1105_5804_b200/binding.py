@@ -20,7 +20,7 @@ NPHASE = 3                                                # SW_NPHASE of include
 SYMBOLS = [
     "sw_create", "sw_destroy", "sw_workspace_bytes", "sw_bind", "sw_set_threshold", "sw_get_threshold",
     "sw_set_counter", "sw_get_counter", "sw_init_spins", "sw_sweep", "sw_activate", "sw_label",
-    "sw_cluster_stats", "wolff_step", "sw_observables", "sw_observables_ex", "sw_series_read", "sw_wolff_frontier", "sw_sweep_host", "sw_launch_count", "sw_strerror",
+    "sw_cluster_stats", "wolff_step", "sw_observables", "sw_observables_ex", "sw_series_read", "sw_wolff_frontier", "sw_sweep_host", "sw_sweep_host_ex", "sw_launch_count", "sw_strerror",
     "sw_last_cuda_error", "sw_profile_enable", "sw_profile_read", "sw_create3d", "sw_workspace_bytes3d", "sw_label_paper",
     "sw_set_band", "sw_band_layout", "sw_sweep_band_begin", "sw_sweep_band_end", "sw_band_counters",
 ]
@@ -98,6 +98,7 @@ def lib():
     L.sw_wolff_frontier.argtypes = [vp, C.c_int]
     L.sw_series_read.argtypes = [vp, u64, i64, C.POINTER(i64), C.POINTER(i64), vp]
     L.sw_sweep_host.argtypes = [vp, vp, i64, vp, vp, C.POINTER(sw_obs), vp]
+    L.sw_sweep_host_ex.argtypes = [vp, vp, i64, vp, vp, C.POINTER(sw_obs), C.c_int, vp]
     L.sw_launch_count.argtypes = [vp, C.POINTER(u64)]
     L.sw_profile_enable.argtypes = [vp, C.c_int]
     L.sw_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(u64)]
@@ -259,14 +260,15 @@ class Lattice:
         self._check(self._lib.sw_series_read(self._h, t_first, n, E, M, self._stream()))
         return list(E), (list(M) if magnetisation else None)
 
-    def sweep_host(self, h_spins_in, n: int, h_spins_out=None, h_labels_out=None, want_obs: bool = True):
+    def sweep_host(self, h_spins_in, n: int, h_spins_out=None, h_labels_out=None, want_obs: bool = True,
+                   obs_flags: int = OBS_SPINS | OBS_CLUSTERS):
         """Host-buffer end-to-end call: torch CPU tensors (ideally pinned) in and out."""
         out = sw_obs()
-        self._check(self._lib.sw_sweep_host(
+        self._check(self._lib.sw_sweep_host_ex(
             self._h, h_spins_in.data_ptr() if h_spins_in is not None else None, n,
             h_spins_out.data_ptr() if h_spins_out is not None else None,
             h_labels_out.data_ptr() if h_labels_out is not None else None,
-            C.byref(out) if want_obs else None, self._stream()))
+            C.byref(out) if want_obs else None, obs_flags, self._stream()))
         return out.as_dict() if want_obs else None
 
     def profile_enable(self, on: bool):

@@ -947,6 +947,12 @@ int sw_series_read(sw_handle* h, uint64_t t_first, int64_t n, int64_t* h_energy,
 int sw_sweep_host(sw_handle* h, const void* h_spins_in, int64_t n, void* h_spins_out, int32_t* h_labels_out,
                   sw_obs* h_obs, void* stream)
 {
+    return sw_sweep_host_ex(h, h_spins_in, n, h_spins_out, h_labels_out, h_obs, SW_OBS_SPINS | SW_OBS_CLUSTERS, stream);
+}
+
+int sw_sweep_host_ex(sw_handle* h, const void* h_spins_in, int64_t n, void* h_spins_out, int32_t* h_labels_out,
+                     sw_obs* h_obs, int obs_flags, void* stream)
+{
     if (!h || n < 0) return SW_EINVAL;
     if (!h->bound) return SW_ESTATE;
     DeviceGuard guard(h);
@@ -957,7 +963,7 @@ int sw_sweep_host(sw_handle* h, const void* h_spins_in, int64_t n, void* h_spins
     if (h_spins_out) SW_CUDA(h, cudaMemcpyAsync(h_spins_out, h->d_spins, (size_t)h->N, cudaMemcpyDeviceToHost, s));
     if (h_labels_out)
         SW_CUDA(h, cudaMemcpyAsync(h_labels_out, h->d_labels, (size_t)h->N * sizeof(int32_t), cudaMemcpyDeviceToHost, s));
-    if (h_obs) return sw_observables(h, h_obs, stream);
+    if (h_obs) return sw_observables_ex(h, h_obs, obs_flags, stream);
     SW_CUDA(h, cudaStreamSynchronize(s));
     return SW_OK;
 }

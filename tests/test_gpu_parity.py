@@ -246,6 +246,15 @@ def test_sweep_host_end_to_end():
         lab, _, nc, nb = oracle.sweep(L, 2, lat.get_threshold(), seed, t, s)
     assert np.array_equal(h_out.numpy(), s) and np.array_equal(h_lab.numpy(), lab)
     assert o["energy"] == oracle.observables(L, 2, s)["energy"] and o["n_clusters"] == nc
+    assert o["max_cluster"] == oracle.cluster_stats(lab)["max_cluster"]
+    # the cheap variant: spin part and the labelling's own counters, no cluster-size pass
+    h_in.copy_(h_out)
+    o2 = lat.sweep_host(h_in, 1, h_out, None, obs_flags=binding.OBS_SPINS)
+    lab, _, nc, nb = oracle.sweep(L, 2, lat.get_threshold(), seed, 3, s)
+    w = oracle.observables(L, 2, s)
+    assert np.array_equal(h_out.numpy(), s)
+    assert o2["energy"] == w["energy"] and o2["magnetisation"] == w["magnetisation"]
+    assert o2["n_clusters"] == nc and o2["n_active_bonds"] == nb and o2["max_cluster"] == 0
     lat.close()
 
 
