@@ -343,3 +343,26 @@ def test_wolff_frontier_growth_matches_the_oracle(L, beta, levels, nsteps):
     sz, i0, root = oracle.wolff_step(L, T, seed, t0 + nsteps + 9, s)
     assert sizes == [sz] and lat.labels_host()[i0] == root and np.array_equal(lat.spins_host(), s)
     lat.close()
+
+
+def test_sweeps_on_a_side_stream_and_two_handles_interleaved():
+    """The kernels of a sweep are chained by programmatic dependent launch: the chain must hold on a non-default stream and
+    when the launches of two handles alternate on one stream."""
+    L, q = 260, 2
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        a = binding.Lattice(L, q, BETA_C, 11)
+        b = binding.Lattice(L, q, 0.5, 12)
+        a.init_spins(1); b.init_spins(1)
+        for _ in range(4):
+            a.sweep(1); b.sweep(1); a.sweep(1)
+        side.synchronize()
+        for lat, seed, n in ((a, 11, 8), (b, 12, 4)):
+            s = oracle.init_spins(L, q, seed, 1)
+            lab = None
+            for t in range(n):
+                lab, _, nc, nb = oracle.sweep(L, q, lat.get_threshold(), seed, t, s)
+            assert np.array_equal(lat.spins_host(), s) and np.array_equal(lat.labels_host(), lab)
+            o = lat.observables(spins=False, clusters=False)
+            assert o["n_clusters"] == nc and o["n_active_bonds"] == nb
+        a.close(); b.close()
