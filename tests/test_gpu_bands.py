@@ -106,3 +106,28 @@ def test_band_arguments_and_states():
     l2 = binding.Lattice(100, 2, 0.4, 1)
     assert lib.sw_set_band(l2._h, 0, 2) == binding.SW_EINVAL           # L must be a multiple of the strip height
     l2.close()
+
+
+def test_L16384_four_bands_equilibrated_vs_single_gpu_and_oracle():
+    """Full size: the equilibrated critical L=16384 state (giant cluster through every band) handed to 4 bands; 3 sweeps must
+    equal the single-GPU chain bit for bit, the last one is also checked against the oracle from the same state."""
+    L, q, seed, G = 16384, 2, 1, 4
+    ref = binding.Lattice(L, q, BETA_C, seed)
+    ref.init_spins(1)
+    ref.sweep(60)
+    grp = bands.BandGroup(L, q, BETA_C, seed, G)
+    for lat in grp.lats:
+        lat.spins.copy_(ref.spins)
+        lat.set_counter(ref.get_counter())
+    grp.sweep(2); ref.sweep(2)
+    assert np.array_equal(grp.spins_host(), ref.spins_host())
+    s = ref.spins_host().copy()
+    t = ref.get_counter()
+    grp.sweep(1); ref.sweep(1)
+    got_s, got_l = grp.spins_host(), grp.labels_host()
+    assert np.array_equal(got_s, ref.spins_host()) and np.array_equal(got_l, ref.labels_host())
+    lab, _, nc, nb = oracle.sweep(L, q, ref.get_threshold(), seed, t, s)
+    assert np.array_equal(got_l, lab) and np.array_equal(got_s, s)
+    c = grp.counters()
+    assert c["n_clusters"] == nc and c["n_active_bonds"] == nb
+    grp.close(); ref.close()
