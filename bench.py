@@ -228,6 +228,52 @@ def run_ablation(args):
     return 0
 
 
+# ------------------------------------------------------------------------------------------------ the other BASELINE.json configs
+def per_config_leg(binding, torch, device):
+    """ns per spin update of the BASELINE.json configs that are not the headline (north_star: "ns/spin-update reported per
+    config"): configs[0] L=64, configs[1] L=1024 cold, configs[3] percolation labelling at p = 0.3 / 0.7, configs[4] q=4 Potts
+    L=4096 and Wolff steps on L=4096.  Small lattices are latency bound, not a roofline statement."""
+    stream = torch.cuda.current_stream()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+    def timed(fn, n):
+        torch.cuda.synchronize(); ev0.record(stream); fn(n); ev1.record(stream); torch.cuda.synchronize()
+        return ev0.elapsed_time(ev1) / n
+
+    out = {}
+    for name, L, q, beta, mode, equil, n in (("configs[0] 2D Ising L=64 beta_c", 64, 2, beta_c_ising(), 1, 100, 1000),
+                                             ("configs[1] 2D Ising L=1024 beta_c cold start", 1024, 2, beta_c_ising(), 0, 100, 900),
+                                             ("configs[4] q=4 Potts L=4096 beta_c=ln 3", 4096, 4, math.log(3.0), 1, 100, 400)):
+        lat = binding.Lattice(L, q, beta, 1, device=device)
+        lat.init_spins(mode); lat.sweep(equil)
+        ms = timed(lat.sweep, n)
+        o = lat.observables(clusters=False)
+        out[name] = {"ms_per_sweep": ms, "ns_per_spin_update": ms * 1e6 / (L * L), "sweeps": n,
+                     "energy_per_site": o["energy"] / (L * L)}
+        lat.close()
+    L = 4096
+    lat = binding.Lattice(L, 2, beta_c_ising(), 1, device=device)
+    lat.init_spins(1); lat.sweep(200)
+    torch.cuda.synchronize(); ev0.record(stream); sizes = lat.wolff_step(500); ev1.record(stream); torch.cuda.synchronize()
+    ms = ev0.elapsed_time(ev1) / 500
+    out["configs[4] Wolff steps, 2D Ising L=4096 beta_c (label everything)"] = {
+        "ms_per_step": ms, "mean_cluster_sites": sum(sizes) / 500.0, "ns_per_cluster_site": ms * 1e6 / max(1.0, sum(sizes) / 500.0)}
+    lat.close()
+    L = 16384
+    latp = binding.Lattice(L, 2, 0.1, 1, device=device, with_bonds=True)
+    latp.init_spins(0)
+    for pbond in (0.3, 0.7):
+        latp.set_threshold(int(pbond * 4294967296.0))
+        latp.activate(); latp.label()
+        ms = timed(lambda n: [latp.label() for _ in range(n)], 10)
+        cs = latp.cluster_stats()
+        out["configs[3] bond percolation labelling L=16384 p=%.1f" % pbond] = {
+            "ms": ms, "ns_per_site": ms * 1e6 / (L * L), "GB/s": BYTES_PER_SITE_LABEL * L * L / (ms * 1e-3) / 1e9,
+            "clusters_per_site": cs["n_clusters"] / (L * L), "largest_cluster_fraction": cs["max_cluster"] / (L * L)}
+    latp.close()
+    return out
+
+
 # ------------------------------------------------------------------------------------------------ simple cubic lattice
 def cubic_leg(binding, torch, device, sizes):
     """SW sweeps of the 3D Ising model at its critical coupling on L^3 periodic lattices: (L, timed sweeps) per entry."""
@@ -478,6 +524,8 @@ def run_ours(args):
     # ---- simple cubic lattice: a second workload, 3D Ising at its critical coupling ------------------
     cubic = cubic_leg(binding, torch, device, ((256, 50), (512, 20))) if rank == 0 and not args.no_cubic else None
 
+    per_config = per_config_leg(binding, torch, device) if rank == 0 and not args.no_per_config else None
+
     # ---- end to end through the host-buffer entry point ----------------------------------------------------
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
     h_in = torch.empty(N, dtype=torch.int8).pin_memory()
@@ -575,6 +623,7 @@ def run_ours(args):
         "labelling": labelling,
         "other_betas": other_betas,
         "cubic": cubic,
+        "per_config": per_config,
         "state_before_timed_region": state_before,
         "state": state_after,
     }
@@ -599,6 +648,7 @@ def main(argv=None):
     ap.add_argument("--bands", action="store_true", help="with --gpus N under torchrun: one lattice in N row bands (strong scaling) instead of N replicas")
     ap.add_argument("--bands-one-gpu", type=int, default=0, metavar="G", help="time the G-band algorithm band after band on one GPU next to sw_sweep")
     ap.add_argument("--ablation", action="store_true", help="time the paper's own labelling pipeline next to sw_label (SURVEY 8(f) row 4)")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the legs of the other BASELINE.json configs")
     ap.add_argument("--only-cubic", action="store_true", help="run the L=256 simple cubic leg alone (ncu captures of the k3_* kernels)")
     ap.add_argument("--no-cubic", action="store_true", help="skip the simple cubic lattice legs (SURVEY 8(f) row 2)")
     ap.add_argument("--no-other-betas", action="store_true", help="skip the beta = 0.40 / 0.50 legs of BASELINE.json configs[2]")
