@@ -143,44 +143,34 @@ k3_local(const Params p, const uint32_t* __restrict__ spins_w, int* __restrict__
             nact += __popc(b);
         }
         s_bnd[l >> 2] = b;
-        // the runs along x inside the word are linked right away: a site points to the first site of its run
-        const int l1 = (b & 0x00000001u) ? l : l + 1, l2 = (b & 0x00000100u) ? l1 : l + 2, l3 = (b & 0x00010000u) ? l2 : l + 3;
-        *reinterpret_cast<int4*>(&s_lab[l]) = make_int4(l, l1, l2, l3);
+        // the runs along x are labelled right here, without a union: inside the word by the bond bits; across the 8 words of a
+        // tile row (8 neighbouring lanes) by a segmented scan -- a word that is one run and linked to its left neighbour
+        // passes that neighbour's outgoing root on -- so that every site starts pointing at the first site of its x-run
+        const bool e0 = b & 0x00000001u, e1 = b & 0x00000100u, e2 = b & 0x00010000u;
+        const bool e3 = (b & 0x01000000u) && 4 * wx + 4 < c.ex;
+        const bool link_in = __shfl_up_sync(FULLM, e3, 1, C3X / 4) && wx > 0;
+        int val = e2 ? (e1 ? (e0 ? l : l + 1) : l + 2) : l + 3;     // first site of the run that leaves the word to the right
+        bool pass = e0 && e1 && e2 && link_in;
+#pragma unroll
+        for (int d = 1; d < C3X / 4; d <<= 1) {
+            const int v = __shfl_up_sync(FULLM, val, d, C3X / 4);
+            const bool q = __shfl_up_sync(FULLM, pass, d, C3X / 4);
+            if (pass && wx >= d) { val = v; pass = q; }
+        }
+        const int rin = __shfl_up_sync(FULLM, val, 1, C3X / 4);
+        const int f0 = link_in ? rin : l;
+        const int l1 = e0 ? f0 : l + 1, l2 = e1 ? l1 : l + 2, l3 = e2 ? l2 : l + 3;
+        *reinterpret_cast<int4*>(&s_lab[l]) = make_int4(f0, l1, l2, l3);
     }
     __syncthreads();
-    // (2) unions over the bonds that stay inside the tile.  East: the links between the words of a row, then every site is
-    // pointed at the root of its x-run.  North, then up: a thread WALKS a line of sites (north: fixed x and z, y = 0 .. C3Y-1,
-    // a warp per plane; up: fixed x and y, z = 0 .. C3Z-1, a warp per row) and carries the root of the set it is in: where the
+    // (2) unions over the bonds that stay inside the tile (the x-runs are labelled already).  North, then up: a thread WALKS
+    // a line of sites (north: fixed x and z, y = 0 .. C3Y-1, a warp per plane; up: fixed x and y, z = 0 .. C3Z-1, a warp per row) and carries the root of the set it is in: where the
     // bond to the next site is active that site's tree is united with the carried root (one side of the union needs no
     // find, and sets are joined bottom-up, so the trees stay shallow); where it is not, the walk continues with the next
     // site's root.  Unions are lock-free (other lanes walk the neighbouring lines at the same time): atomicMin hook of the
     // larger root under the smaller.  (One union per bond position of a word, direction by direction: 0.239 ms at L = 256;
     // the walks: see DESIGN.md.)
     static_assert(C3X == 32 && C3THREADS == C3X * C3Y && C3THREADS == C3X * C3Z, "one lane per x, one warp per plane / row");
-#pragma unroll
-    for (int k = 0; k < C3ITEMS; ++k) {
-        const int item = threadIdx.x + k * C3THREADS;
-        const int wx = item % (C3X / 4), r = item / (C3X / 4), ly = r % C3Y, lz = r / C3Y;
-        const int l = (lz * C3Y + ly) * C3X + 4 * wx;
-        if ((s_bnd[l >> 2] & 0x01000000u) && 4 * wx + 4 < c.ex) unite_s(s_lab, l + 3, l + 4);
-    }
-    __syncthreads();
-    {
-        int rt[C3ITEMS][4];
-#pragma unroll
-        for (int k = 0; k < C3ITEMS; ++k) {
-            const int l = 4 * (threadIdx.x + k * C3THREADS);
-#pragma unroll
-            for (int j = 0; j < 4; ++j) rt[k][j] = find_s(s_lab, l + j);
-        }
-        __syncthreads();
-#pragma unroll
-        for (int k = 0; k < C3ITEMS; ++k) {
-            const int l = 4 * (threadIdx.x + k * C3THREADS);
-            *reinterpret_cast<int4*>(&s_lab[l]) = make_int4(rt[k][0], rt[k][1], rt[k][2], rt[k][3]);
-        }
-    }
-    __syncthreads();
     const uint8_t* const s_bb = reinterpret_cast<const uint8_t*>(s_bnd);
 #pragma unroll
     for (int dir = 1; dir < 3; ++dir) {
@@ -219,7 +209,8 @@ k3_local(const Params p, const uint32_t* __restrict__ spins_w, int* __restrict__
             int g[4];
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
-                const int rt = find_s(s_lab, l + j);
+                int rt = l + j, pp = s_lab[rt];          // (read-only chase: the trees are shallow and final)
+                while (pp != rt) { rt = pp; pp = s_lab[rt]; }
                 const int rx = rt % C3X, rr = rt / C3X, ry = rr % C3Y, rz = rr / C3Y;
                 g[j] = ((c.z0 + rz) * L + (c.y0 + ry)) * L + c.x0 + rx;
             }
