@@ -408,7 +408,12 @@ uint64_t orc_fnv1a64(const uint8_t *p, int64_t n)
  * independent transitive closure and scipy's connected components, wrap bonds in all
  * three directions; orc3_observables -- numpy definition, closed forms (cold, layered);
  * orc3_sweep / orc3_run_chain -- exact <E>, <|m|>, <m^2> of the 3 x 3 x 3 Ising model
- * (sum over all 2^27 states, done plane by plane in the test) and the FK identity.
+ * (sum over all 2^27 states, done plane by plane in the test) and the FK identity;
+ * orc3_init_spins -- equals orc_init_spins at equal N (golden L4_init_k pins that one)
+ * and the keying (i>>2, 0, 0, INIT)[i&3] rebuilt from the KAT-pinned Philox;
+ * orc3_flip -- constant on clusters, k_r rebuilt per root from the pinned Philox with
+ * both words of t in use, Ising storage (a slipped counter word, word index or domain
+ * in either function fails these).
  * ================================================================================== */
 enum { DOM_BOND3 = 4 };
 

@@ -188,3 +188,50 @@ def test_chain3_against_exact_3x3x3(beta):
     e, mm = ser[:, 0] / N, ser[:, 1] / N
     for got, want in ((e, e_ex), (np.abs(mm), mabs_ex), (mm * mm, m2_ex), (ser[:, 3] / float(N * N), m2_ex)):   # last: FK identity
         assert abs(got.mean() - want) < 4.5 * blocked_error(got) + 1e-12
+
+
+def test_init_spins3_is_the_2d_definition_over_N_sites_keyed_by_quad():
+    """orc3_init_spins (S:8c.8 over N = L^3 sites, reading 19): k_i = (PHILOX(seed; i>>2, 0, 0, INIT=0)[i&3] q) >> 32.
+    Pinned (a) to the 2D function at equal N (its own pin is the survey's golden L4_init_k) and (b) to the keying rebuilt from
+    the KAT-pinned Philox primitive; a slip in the counter word (i>>1 for i>>2), the word index or the domain fails both."""
+    for q, seed in ((2, 11), (3, 2 ** 40 + 7), (8, 5)):
+        key = [seed & 0xFFFFFFFF, seed >> 32]
+        s3 = oracle.init_spins3(4, q, seed, 1)                          # N = 64
+        s2 = oracle.init_spins(8, q, seed, 1)                           # N = 64
+        assert s3.shape == (64,) and np.array_equal(s3, s2)
+        k3 = (1 - s3.astype(np.int64)) // 2 if q == 2 else s3.astype(np.int64)
+        want = [(int(oracle.philox([i >> 2, 0, 0, 0], key)[i & 3]) * q) >> 32 for i in range(64)]
+        assert k3.tolist() == want
+        assert len(set(want)) > 1
+        # a larger, non-power-of-two lattice through the primitive only
+        s3 = oracle.init_spins3(6, q, seed, 1)
+        k3 = (1 - s3.astype(np.int64)) // 2 if q == 2 else s3.astype(np.int64)
+        assert k3.tolist() == [(int(oracle.philox([i >> 2, 0, 0, 0], key)[i & 3]) * q) >> 32 for i in range(216)]
+        cold = oracle.init_spins3(5, q, seed, 0)
+        assert (cold == (1 if q == 2 else 0)).all()
+
+
+def test_flip3_is_constant_on_clusters_and_keyed_by_root():
+    """orc3_flip (P:55 step 3; S:8c.6): every site takes k_r = (PHILOX(seed; r, t_lo, t_hi, FLIP=2)[0] q) >> 32 of its root r.
+    The 3D twin of test_flip_is_constant_on_clusters_and_keyed_by_root, with the step counter's high word in use."""
+    L, q, seed = 6, 4, 77 + (3 << 32)
+    t = (5 << 32) + 9
+    rng = np.random.default_rng(12)
+    codes = (rng.random((L ** 3, 3)) < 0.22)
+    codes = (codes[:, 0] | (codes[:, 1] << 1) | (codes[:, 2] << 2)).astype(np.uint8)
+    lab, nc = oracle.label3(L, codes)
+    assert 1 < nc < L ** 3
+    key = [seed & 0xFFFFFFFF, seed >> 32]
+    s = oracle.flip3(q, seed, t, lab)
+    assert np.array_equal(s, s[lab]) and s.min() >= 0 and s.max() < q
+    roots = np.unique(lab)
+    for r in roots:
+        w = oracle.philox([int(r), t & 0xFFFFFFFF, t >> 32, 2], key)
+        assert s[r] == (int(w[0]) * q) >> 32
+    assert not np.array_equal(s, oracle.flip3(q, seed, t + 1, lab))
+    assert not np.array_equal(s, oracle.flip3(q, seed, t + (1 << 32), lab))      # the high word of t is part of the counter
+    s2 = oracle.flip3(2, seed, t, lab)                                  # Ising storage: k=0 -> +1, k=1 -> -1
+    assert set(np.unique(s2)) <= {-1, 1}
+    for r in roots:
+        w = oracle.philox([int(r), t & 0xFFFFFFFF, t >> 32, 2], key)
+        assert s2[r] == (1 if (int(w[0]) >> 31) == 0 else -1)
