@@ -42,7 +42,8 @@ enum {
                          misaligned pointer, workspace too small, n<0                                      */
     SW_ESTATE  = -2,  /* handle not bound (sw_bind not called), or d_bonds needed but bound as NULL        */
     SW_ECUDA   = -3,  /* a CUDA runtime call or kernel launch failed; text via sw_strerror / sw_last_cuda_error */
-    SW_ENOMEM  = -4   /* host allocation failed                                                          */
+    SW_ENOMEM  = -4,  /* host allocation failed                                                          */
+    SW_ELIMIT  = -5   /* sw_cluster_stats_static: the lattice has more than SW_STATIC_MAX_SITES sites        */
 };
 
 typedef struct sw_handle sw_handle;   /* opaque; host-side state only */
@@ -144,6 +145,34 @@ int sw_label(sw_handle* h, const uint8_t* d_bonds_in, int32_t* d_labels_out, voi
 
 /* Cluster statistics of canonical labels (d_labels_in == NULL: the bound d_labels).  Synchronises `stream`. */
 int sw_cluster_stats(sw_handle* h, const int32_t* d_labels_in, sw_cstats* h_out, void* stream);
+
+/* Cluster statistics WITHOUT a workspace, for callers that cannot obtain device memory at the moment they need the numbers.
+ * sw_cluster_stats needs a bound handle, i.e. a d_work of sw_workspace_bytes() that somebody had to allocate (4 bytes per site
+ * of cluster-size scratch plus the strip arrays).  Some users of this library cannot do that: a measurement hook that runs
+ * inside a simulation whose device memory is entirely handed out to a pool of fixed size (a raw cudaMalloc there fails, or
+ * steals pages the pool expects to get back); a latency-critical loop, where cudaMalloc / cudaFree synchronise the whole
+ * device; a plug-in that is handed two device pointers and nothing else.  For them the per-root size array and the
+ * accumulators live in ONE array compiled into the library (`static __device__`, SW_STATIC_MAX_SITES int32 + 4 KiB,
+ * about 4 MiB): every GPU that loads libswb200.so holds that much from the moment the library's module is loaded on it
+ * until the process exits, whether or not this function is ever called.
+ *   L        : L x L square lattice, 4 <= L, L % 4 == 0, L * L <= SW_STATIC_MAX_SITES (L <= 1024); a larger lattice is refused
+ *              with SW_ELIMIT and nothing is launched (use sw_cluster_stats with a workspace).
+ *   d_labels : DEVICE, N = L * L int32, 16-byte aligned, canonical labels (every value the index of a site, e.g. what
+ *              sw_sweep / sw_label wrote); read only.
+ *   d_out    : DEVICE, one sw_cstats, 8-byte aligned, on the same GPU as d_labels; overwritten.  Valid once `stream` has
+ *              reached the end of the call's work; the call itself is asynchronous and copies nothing to the host.
+ * The call allocates nothing: no cudaMalloc / cudaFree, no allocating library routine, no host heap.  It needs no handle.
+ * The GPU d_labels lives on is made current for the duration of the call.  The FIRST call on each GPU also looks up the
+ * device address of the array on that GPU (cudaGetSymbolAddress, once per device; the result is cached); make that first call
+ * at set-up time, before any stream capture begins.
+ * The array is shared by every call in the process and keeps whatever the previous call left, so each call first clears the
+ * part it uses, on `stream`.  Two calls whose work overlaps on one GPU (different streams, or different host threads on different
+ * streams) race on it and both results are garbage: order them on one stream or with events.  Calls on different GPUs do not
+ * interact (each GPU has its own copy).
+ * Errors: SW_EINVAL (NULL / misaligned pointer, bad L, a pointer that is not device memory, d_out on another GPU), SW_ELIMIT
+ * (lattice larger than the array), SW_ECUDA (a runtime call or launch failed). */
+#define SW_STATIC_MAX_SITES (1 << 20)
+int sw_cluster_stats_static(int32_t L, const int32_t* d_labels, sw_cstats* d_out, void* stream);
 
 /* ABLATION BASELINE (S:8f row 4): the same labelling as sw_label, computed the way the PAPER does it -- self-labelling on
  * B x B tiles in shared memory, then tile consolidation by label relaxation (method 0) or by

@@ -12,7 +12,8 @@ from typing import Optional
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libswb200.so")
 
-SW_OK, SW_EINVAL, SW_ESTATE, SW_ECUDA, SW_ENOMEM = 0, -1, -2, -3, -4
+SW_OK, SW_EINVAL, SW_ESTATE, SW_ECUDA, SW_ENOMEM, SW_ELIMIT = 0, -1, -2, -3, -4, -5
+STATIC_MAX_SITES = 1 << 20                                # SW_STATIC_MAX_SITES of include/swb200.h
 OBS_SPINS, OBS_CLUSTERS = 1, 2                            # SW_OBS_* of include/swb200.h
 NPHASE = 3                                                # SW_NPHASE of include/swb200.h
 
@@ -23,6 +24,7 @@ SYMBOLS = [
     "sw_cluster_stats", "wolff_step", "sw_observables", "sw_observables_ex", "sw_series_read", "sw_wolff_frontier", "sw_sweep_host", "sw_sweep_host_ex", "sw_launch_count", "sw_strerror",
     "sw_last_cuda_error", "sw_profile_enable", "sw_profile_read", "sw_create3d", "sw_workspace_bytes3d", "sw_label_paper",
     "sw_set_band", "sw_band_layout", "sw_sweep_band_begin", "sw_sweep_band_end", "sw_band_counters",
+    "sw_cluster_stats_static",
 ]
 
 
@@ -85,6 +87,7 @@ def lib():
     L.sw_activate.argtypes = [vp, vp]
     L.sw_label.argtypes = [vp, vp, vp, vp]
     L.sw_cluster_stats.argtypes = [vp, vp, C.POINTER(sw_cstats), vp]
+    L.sw_cluster_stats_static.argtypes = [i32, vp, vp, vp]
     L.sw_label_paper.argtypes = [vp, C.c_int, C.c_int, vp, vp, C.POINTER(sw_paper_stats), vp]
     L.sw_set_band.argtypes = [vp, C.c_int, C.c_int]
     L.sw_band_layout.argtypes = [vp, C.c_int, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), C.POINTER(C.c_size_t),
@@ -118,6 +121,30 @@ class SwError(RuntimeError):
         self.code = code
         msg = lib().sw_strerror(code).decode()
         super().__init__("swb200: %s (%d)%s" % (msg, code, (": " + detail) if detail else ""))
+
+
+def cluster_stats_static(L: int, labels, out=None) -> "object":
+    """sw_cluster_stats_static: cluster statistics of an L x L label tensor with no workspace and no handle, for callers that
+    cannot allocate device memory (the scratch is an array built into the library; L * L <= STATIC_MAX_SITES).
+
+    labels: int32 CUDA tensor of L * L canonical labels.  out: a CUDA tensor of >= 35 int64 on the same GPU that receives the
+    sw_cstats (n_clusters, max_cluster, sum_sq_cluster, hist32[32]); if None one is created here (which allocates -- pass your
+    own to stay allocation-free).  Asynchronous on torch's current stream of that GPU; returns `out`.  Calls that overlap on
+    one GPU race on the shared array."""
+    import torch
+    if out is None:
+        out = torch.empty(C.sizeof(sw_cstats) // 8, dtype=torch.int64, device=labels.device)
+    stream = C.c_void_p(torch.cuda.current_stream(labels.device).cuda_stream)
+    rc = lib().sw_cluster_stats_static(L, labels.data_ptr(), out.data_ptr(), stream)
+    if rc != SW_OK:
+        raise SwError(rc)
+    return out
+
+
+def cstats_from_tensor(out) -> dict:
+    """The sw_cstats a cluster_stats_static call left in `out`, as the dict Lattice.cluster_stats returns (synchronising copy)."""
+    v = out.cpu().tolist()
+    return {"n_clusters": v[0], "max_cluster": v[1], "sum_sq_cluster": v[2] & 0xFFFFFFFFFFFFFFFF, "hist32": v[3:35]}
 
 
 class Lattice:

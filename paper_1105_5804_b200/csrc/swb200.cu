@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include "common.cuh"
@@ -302,6 +303,7 @@ const char* sw_strerror(int code)
         case SW_ESTATE: return "handle not bound, or a needed buffer was bound as NULL";
         case SW_ECUDA: return "CUDA error (see sw_last_cuda_error)";
         case SW_ENOMEM: return "out of host memory";
+        case SW_ELIMIT: return "lattice larger than the built-in scratch array (SW_STATIC_MAX_SITES sites): use sw_cluster_stats with a workspace";
         default: return "unknown error code";
     }
 }
@@ -969,3 +971,88 @@ int sw_sweep_host_ex(sw_handle* h, const void* h_spins_in, int64_t n, void* h_sp
 }
 
 }  // extern "C"
+
+// ---- sw_cluster_stats_static: cluster statistics with the scratch compiled into the library (include/swb200.h) -----------
+// For callers that cannot allocate device memory (see the header).  Everything the two cluster kernels need beyond the labels
+// and the result -- the accumulators and one int32 per site -- lives in the array below.  Its name is only a handle on the
+// host side: the kernels get the device address that cudaGetSymbolAddress returns for the GPU that is current, looked up once
+// per GPU.  Nothing here calls cudaMalloc, cudaFree or an allocating routine.
+namespace {
+
+constexpr int STATIC_ACC_INTS = (int)((sizeof(Acc) + 255) / 256 * 256 / sizeof(int));   // the Acc, padded to 256 bytes
+static_assert(STATIC_ACC_INTS * sizeof(int) >= sizeof(Acc), "the accumulators fit in front of the size array");
+static __device__ __align__(256) int g_static_scratch[STATIC_ACC_INTS + SW_STATIC_MAX_SITES];
+
+constexpr int STATIC_MAX_DEVICES = 64;
+std::mutex g_static_mutex;                                // guards the table below (first calls from several host threads)
+int* g_static_ptr[STATIC_MAX_DEVICES];                    // device address of g_static_scratch on GPU d; NULL: not looked up yet
+
+// accumulators of k_cluster_stats -> the caller's sw_cstats (one warp; bin b by lane b)
+__global__ void k_cstats_emit(const Acc* __restrict__ acc, sw_cstats* __restrict__ out)
+{
+    out->hist32[threadIdx.x] = (int64_t)acc->hist[threadIdx.x];
+    if (threadIdx.x == 0) {
+        out->n_clusters = (int64_t)acc->cs_nclusters;
+        out->max_cluster = (int64_t)acc->cs_max;
+        out->sum_sq_cluster = acc->cs_sumsq;
+    }
+}
+
+}  // namespace
+
+extern "C" int sw_cluster_stats_static(int32_t L, const int32_t* d_labels, sw_cstats* d_out, void* stream)
+{
+    if (L < 4 || (L % 4) != 0 || !d_labels || !d_out) return SW_EINVAL;
+    if (((uintptr_t)d_labels & 15u) || ((uintptr_t)d_out & 7u)) return SW_EINVAL;
+    const int64_t N = (int64_t)L * L;
+    if (N > (int64_t)SW_STATIC_MAX_SITES) return SW_ELIMIT;
+    cudaPointerAttributes at_in, at_out;
+    if (cudaPointerGetAttributes(&at_in, d_labels) != cudaSuccess || cudaPointerGetAttributes(&at_out, d_out) != cudaSuccess) {
+        cudaGetLastError();
+        return SW_EINVAL;
+    }
+    const bool dev_in = at_in.type == cudaMemoryTypeDevice || at_in.type == cudaMemoryTypeManaged;
+    const bool dev_out = at_out.type == cudaMemoryTypeDevice || at_out.type == cudaMemoryTypeManaged;
+    if (!dev_in || !dev_out || at_in.device != at_out.device) return SW_EINVAL;
+    const int dev = at_in.device;
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) return SW_EINVAL;
+    // make the GPU of the buffers current for the call (as every handle entry point does), restore the caller's afterwards
+    struct Current {
+        int prev = -1; bool switched = false;
+        ~Current() { if (switched) cudaSetDevice(prev); }
+    } cur;
+    if (cudaGetDevice(&cur.prev) != cudaSuccess) return SW_ECUDA;
+    if (cur.prev != dev) {
+        if (cudaSetDevice(dev) != cudaSuccess) return SW_ECUDA;
+        cur.switched = true;
+    }
+    int* scratch = nullptr;
+    {   // set-up, once per GPU, with that GPU current: the device address of the array (its host-side name is not one)
+        std::lock_guard<std::mutex> lock(g_static_mutex);
+        if (!g_static_ptr[dev]) {
+            void* ptr = nullptr;
+            if (cudaGetSymbolAddress(&ptr, g_static_scratch) != cudaSuccess || !ptr) {
+                cudaGetLastError();
+                return SW_ECUDA;
+            }
+            g_static_ptr[dev] = (int*)ptr;
+        }
+        scratch = g_static_ptr[dev];
+    }
+    Acc* const acc = reinterpret_cast<Acc*>(scratch);
+    int* const size = scratch + STATIC_ACC_INTS;
+    cudaStream_t s = (cudaStream_t)stream;
+    Params p;
+    memset(&p, 0, sizeof(p));
+    p.L = L; p.N = (int32_t)N; p.H = L; p.q = 2; p.logL = -1;
+    p.ntx = (L + TW - 1) / TW; p.nty = (L + TH - 1) / TH; p.nband = p.nty;
+    // the array still holds the previous call's sizes and sums: clear the accumulators and the N entries used now
+    if (cudaMemsetAsync(scratch, 0, ((size_t)STATIC_ACC_INTS + (size_t)N) * sizeof(int), s) != cudaSuccess) return SW_ECUDA;
+    k_cluster_sizes<<<dim3(p.ntx, p.nty), 256, 0, s>>>(p, d_labels, size);
+    if (cudaGetLastError() != cudaSuccess) return SW_ECUDA;
+    k_cluster_stats<<<grid_capped(N, 256, 148 * 8), 256, 0, s>>>(p, d_labels, size, acc);
+    if (cudaGetLastError() != cudaSuccess) return SW_ECUDA;
+    k_cstats_emit<<<1, 32, 0, s>>>(acc, d_out);
+    if (cudaGetLastError() != cudaSuccess) return SW_ECUDA;
+    return SW_OK;
+}
