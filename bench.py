@@ -1,7 +1,8 @@
 #!/usr/bin/env python
 """bench.py -- headline measurement: ns per spin update of a full Swendsen-Wang sweep at L=16384, beta_c, q=2
-(BASELINE.json metric; config 3 at beta_c), on N GPUs of one node as N independent replicas ("replicas only",
-DESIGN.md: the path is specified for one GPU and has no exchange step).
+(BASELINE.json metric; config 3 at beta_c).  --gpus N runs N independent replicas, one per GPU (SURVEY 8(e) "replicas only":
+weak scaling, no data-path collective); --bands instead shards ONE lattice into N row bands with one seam all-gather per sweep
+(strong scaling); --bands-one-gpu G runs that algorithm band after band on one GPU.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--L 16384] [--beta BETA] [--impl ours|reference]
 
@@ -28,6 +29,9 @@ PAPER_NS_L16384 = 3.573          # Table I, Tesla M2070, q=2,
 BYTES_PER_SITE_SWEEP = 14.0      # SURVEY 8(d) model (iii) / DESIGN.md: 1 + 4 + 4 + 4 + 1
 BYTES_PER_SITE = {"k_scan": 5.0, "k_seam": 0.0, "k_final": 9.0}   # DESIGN.md per-kernel table
 PHASES = ["k_scan", "k_seam", "k_final"]
+# bond thresholds floor(p 2^32) of BASELINE.json configs[3], as stored (and pinned) in tests/golden/thresholds.txt -- passed to
+# sw_set_threshold as integers: no method arithmetic in the bench
+PERC_THRESHOLD = {0.3: 1288490188, 0.5: 2147483648, 0.7: 3006477107}
 # ncu counters per launch (dram bytes, warp instructions) are NOT constants of this file: they are read from the tracked
 # capture profiles/r02_counters.json, which records the hash of the kernel sources it was taken on; if the sources have
 # changed since, the fields are reported as null with the reason (ncu_counters below).
@@ -180,7 +184,8 @@ def run_reference(args):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": False,
         "scaling": "weak", "vs_baseline": None, "dtype": "i32", "data": "synthetic",
         "config": {"workload": "2D Ising SW sweep, L=%d periodic, beta=%.10f, q=2" % (args.L, args.beta),
-                   "L": args.L, "q": 2, "beta": args.beta},
+                   "L": args.L, "q": 2, "beta": args.beta, "sampled_L": Ls,
+                   "note": "each timed step is one oracle sweep of an L=%d lattice (a bounded sample of the L=%d workload)" % (Ls, args.L)},
         "cpu_baseline": {"value": ns, "unit": "ns", "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": ns, "unit": "ns", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -220,7 +225,9 @@ def run_ablation(args):
                 st = lat.label_paper(method, B, None, out)
                 rows.append({"L": L, "B": B, "consolidation": "relaxation" if method == 0 else "sewing",
                              "labels_equal_sw_label": bool(torch.equal(out, ref)), "sw_label_ms": ours,
-                             "ms": st["ms_local"] + st["ms_consolidate"] + st["ms_flatten"], **st})
+                             "ms": st["ms_local"] + st["ms_consolidate"] + st["ms_flatten"],
+                             # (the one-thread wrap-around step is this repository's reading of P:213 "in an additional step")
+                             "ms_without_wrap": st["ms_local"] + st["ms_consolidate"] + st["ms_flatten"] - st["ms_wrap"], **st})
         lat.close()
         L *= 2
     print(json.dumps({"ablation": "paper pipeline (P:152-258) vs sw_label, bonds of equilibrated configurations at beta=%.7f" % args.beta,
@@ -263,7 +270,7 @@ def per_config_leg(binding, torch, device):
     latp = binding.Lattice(L, 2, 0.1, 1, device=device, with_bonds=True)
     latp.init_spins(0)
     for pbond in (0.3, 0.7):
-        latp.set_threshold(int(pbond * 4294967296.0))
+        latp.set_threshold(PERC_THRESHOLD[pbond])
         latp.activate(); latp.label()
         ms = timed(lambda n: [latp.label() for _ in range(n)], 10)
         cs = latp.cluster_stats()
@@ -374,6 +381,9 @@ def run_bands_one_gpu(args):
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product has no CPU path")
     L, beta, N, G = args.L, args.beta, args.L * args.L, args.bands_one_gpu
+    if args.steps < 4:
+        raise SystemExit("--bands-one-gpu needs --steps >= 4: three of the group's sweeps are untimed warm-up, the rest are timed")
+    n_timed = args.steps - 3
     ref = binding.Lattice(L, 2, beta, 1)
     ref.init_spins(1); ref.sweep(EQUIL_SWEEPS)
     spins = ref.spins.clone(); t0 = ref.get_counter()
@@ -384,11 +394,12 @@ def run_bands_one_gpu(args):
     for lat in grp.lats:                                  # the same equilibrated state on every band
         lat.spins.copy_(spins); lat.set_counter(t0)
     grp.sweep(3)
-    torch.cuda.synchronize(); ev0.record(); grp.sweep(args.steps - 3); ev1.record(); torch.cuda.synchronize()
-    ms_grp = ev0.elapsed_time(ev1) / max(1, args.steps - 3)
+    torch.cuda.synchronize(); ev0.record(); grp.sweep(n_timed); ev1.record(); torch.cuda.synchronize()
+    ms_grp = ev0.elapsed_time(ev1) / n_timed
     same = bool(torch.equal(torch.from_numpy(grp.spins_host()), ref.spins.cpu()))
     print(json.dumps({"bands_one_gpu": G, "L": L, "beta": beta, "sw_sweep_ms": ms_ref, "all_bands_ms": ms_grp,
                       "per_band_ms": ms_grp / G, "work_inflation": ms_grp / ms_ref,
+                      "sw_sweep_timed_sweeps": args.steps, "bands_timed_sweeps": n_timed, "bands_warmup_sweeps": 3,
                       "spins_equal_single_gpu_chain_after_%d_sweeps" % args.steps: same}), flush=True)
     grp.close(); ref.close()
     return 0

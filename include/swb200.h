@@ -69,6 +69,10 @@ typedef struct {
     int32_t sewing_levels;          /* levels of the hierarchical sewing (log2(L/B)); 0 for relaxation               */
     int32_t reserved;
     double  ms_local, ms_consolidate, ms_flatten;   /* CUDA-event times of the three phases                         */
+    double  ms_wrap;                /* the part of ms_consolidate spent closing the 2L bonds that wrap around the lattice (sewing
+                                       only, else 0).  The paper says only "in an additional step"; here it is ONE thread,
+                                       like the last sewing level -- this repository's choice, reported so that ratios can be
+                                       quoted with and without it                                                     */
 } sw_paper_stats;
 
 /* Cluster statistics of a canonical labelling (S:8a a9; BASELINE.json config 4 "cluster-size histogram"). */
@@ -179,7 +183,8 @@ int sw_cluster_stats_static(int32_t L, const int32_t* d_labels, sw_cstats* d_out
  * hierarchical sewing (method 1), then a flatten pass -- so that the cost of the paper's design on a B200 can be put
  * next to sw_label's.  Output: canonical labels (minimum site index), bit-identical to sw_label's.  B in {8, 16, 32}, L % B == 0,
  * and L / B a power of two for method 1; square lattice only; else SW_EINVAL.  d_bonds_in / d_labels_out as in sw_label.
- * Uses the cluster-size scratch of the workspace.  Synchronises `stream` (the relaxation's stopping criterion is read by the
+ * Uses the cluster-size scratch of the workspace.  The number of active bonds is not counted: a following sw_observables reports
+ * n_active_bonds = 0 (n_clusters is filled).  Synchronises `stream` (the relaxation's stopping criterion is read by the
  * host between launches, as in the paper).  h_stats may be NULL.  Not on the sweep path. */
 int sw_label_paper(sw_handle* h, int method, int B, const uint8_t* d_bonds_in, int32_t* d_labels_out, sw_paper_stats* h_stats,
                    void* stream);

@@ -51,7 +51,8 @@ class sw_cstats(C.Structure):
 
 class sw_paper_stats(C.Structure):
     _fields_ = [("selflabel_passes_max", C.c_int32), ("relax_iterations", C.c_int32), ("sewing_levels", C.c_int32),
-                ("reserved", C.c_int32), ("ms_local", C.c_double), ("ms_consolidate", C.c_double), ("ms_flatten", C.c_double)]
+                ("reserved", C.c_int32), ("ms_local", C.c_double), ("ms_consolidate", C.c_double), ("ms_flatten", C.c_double),
+                ("ms_wrap", C.c_double)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_ if k != "reserved"}

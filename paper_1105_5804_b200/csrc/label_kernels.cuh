@@ -344,7 +344,7 @@ k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __rest
 #pragma unroll
             for (int r = 0; r < GENR; ++r)
                 if (FULL || r < nrow) word |= draw_byte(p, c0 + (uint32_t)r * ((uint32_t)L >> 1), p.u_lo, p.u_hi) << (8 * r);
-            draws[draw_word_index(p, blockIdx.x, blockIdx.y, warp, lane)] = word;
+            draws[draw_word_index(p, blockIdx.x, blockIdx.y + (BAND ? p.ty0 : 0), warp, lane)] = word;   // (ty = the lattice's strip row, as k_scan reads it)
         }
         uint32_t fl = 0;                                 // REF and HOOK bits of the 16 entries
 #pragma unroll

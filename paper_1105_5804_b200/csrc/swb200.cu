@@ -80,7 +80,8 @@ WorkLayout work_layout(int32_t L, int32_t dim)
     w.edgeA = w.series + align_up(sizeof(SeriesEntry) * SERIES_RING);
     w.edgeB = w.edgeA + align_up((ntx + nty) * (size_t)L * sizeof(int32_t));
     w.draws = w.edgeB + align_up((ntx + nty) * (size_t)L * sizeof(int32_t));
-    w.size = w.draws + align_up(ntx * nty * (size_t)(TH / 4) * 32 * sizeof(uint32_t));
+    // (the draw cache exists only in a build with SWB_GEN_ROWS > 0 -- measured and dropped; 64 MiB at L = 16384)
+    w.size = w.draws + align_up(GEN_ROWS > 0 ? ntx * nty * (size_t)(TH / 4) * 32 * sizeof(uint32_t) : 0);
     w.bonds3 = w.size + align_up(N * sizeof(int32_t));
     w.total = w.bonds3 + align_up(dim == 3 ? N : 0);
     return w;
@@ -183,6 +184,25 @@ inline cudaLaunchAttribute pdl_attr()
 }
 #endif
 
+// A kernel that asks for more dynamic shared memory than the 48 KB default needs cudaFuncAttributeMaxDynamicSharedMemorySize
+// raised -- a property of the kernel ON ONE DEVICE.  The (device, kernel) pairs already done are remembered; the default
+// build (SCAN_WARPS = 4: ScanSmem is 37.9 KB) never gets past the first line.  The device of the handle is current here.
+int raise_smem_limit(sw_handle* h, const void* kern, int bytes)
+{
+    if (bytes <= 48 * 1024) return SW_OK;
+    struct Done { int dev; const void* kern; };
+    static std::mutex mtx;
+    static Done done[256];
+    static int ndone = 0;
+    int dev = 0;
+    SW_CUDA(h, cudaGetDevice(&dev));
+    std::lock_guard<std::mutex> lock(mtx);
+    for (int i = 0; i < ndone; ++i) if (done[i].dev == dev && done[i].kern == kern) return SW_OK;
+    SW_CUDA(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    if (ndone < 256) done[ndone++] = Done{dev, kern};    // (a full table only means the attribute is set again next time)
+    return SW_OK;
+}
+
 // labelling of the bond graph of step t (or of packed bonds): k_scan -> k_seam; k_final resolves the rest
 // SRC_PHILOX falls through to SRC_DRAWS when the draw cache holds the draws of step t for the current threshold
 template <int SRC>
@@ -203,13 +223,9 @@ int launch_label_front(sw_handle* h, const Params& p, const uint8_t* bonds, int3
     if (h->nbands > 1)                                   // a row band: L is a multiple of TH, sweeps only (no draw cache)
         kern = ising ? (fullw ? k_scan<SRC_PHILOX, true, true, true> : k_scan<SRC_PHILOX, true, false, true>)
                      : (fullw ? k_scan<SRC_PHILOX, false, true, true> : k_scan<SRC_PHILOX, false, false, true>);
-    static const void* opted[16];                        // kernels whose dynamic shared-memory limit has been raised
-    static int nopted = 0;
-    bool done = false;
-    for (int i = 0; i < nopted; ++i) done = done || opted[i] == (const void*)kern;
-    if (!done) {
-        SW_CUDA(h, cudaFuncSetAttribute((const void*)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(ScanSmem)));
-        if (nopted < 16) opted[nopted++] = (const void*)kern;
+    {
+        const int rc = raise_smem_limit(h, (const void*)kern, (int)sizeof(ScanSmem));
+        if (rc) return rc;
     }
 #if SWB_PDL == 2
     {
@@ -799,11 +815,11 @@ int sw_label_paper(sw_handle* h, int method, int B, const uint8_t* d_bonds_in, i
     int* const d_flag = h->d_wolff_status + 1;           // [0] belongs to the frontier Wolff kernel; [1] changed, [2] passes
     int* const d_rlab = h->d_size;
     struct Events {                                      // destroyed on every return path
-        cudaEvent_t e[4] = {nullptr, nullptr, nullptr, nullptr};
-        ~Events() { for (int k = 0; k < 4; ++k) if (e[k]) cudaEventDestroy(e[k]); }
+        cudaEvent_t e[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // [4]: before the wrap-around step of the sewing
+        ~Events() { for (int k = 0; k < 5; ++k) if (e[k]) cudaEventDestroy(e[k]); }
     } evs;
     cudaEvent_t* const ev = evs.e;
-    for (int k = 0; k < 4; ++k) SW_CUDA(h, cudaEventCreate(&ev[k]));
+    for (int k = 0; k < 5; ++k) SW_CUDA(h, cudaEventCreate(&ev[k]));
     int rc = zero_sweep_counters(h, s);
     if (rc) return rc;
     SW_CUDA(h, cudaMemsetAsync(d_flag, 0, 2 * sizeof(int), s));
@@ -838,6 +854,7 @@ int sw_label_paper(sw_handle* h, int method, int B, const uint8_t* d_bonds_in, i
             SW_LAUNCHED(h, "kp_sew");
             ++levels;
         }
+        SW_CUDA(h, cudaEventRecord(ev[4], s));
         kp_sew_wrap<<<1, 32, 0, s>>>(L, bonds, labels);
         SW_LAUNCHED(h, "kp_sew_wrap");
         SW_CUDA(h, cudaEventRecord(ev[2], s));
@@ -857,6 +874,12 @@ int sw_label_paper(sw_handle* h, int method, int B, const uint8_t* d_bonds_in, i
         h_stats->relax_iterations = iterations;
         h_stats->sewing_levels = levels;
         h_stats->ms_local = t01; h_stats->ms_consolidate = t12; h_stats->ms_flatten = t23;
+        h_stats->ms_wrap = 0.0;
+        if (method == 1) {
+            float tw = 0.f;
+            SW_CUDA(h, cudaEventElapsedTime(&tw, ev[4], ev[2]));
+            h_stats->ms_wrap = tw;
+        }
     }
     h->last_labels = labels;
     return SW_OK;

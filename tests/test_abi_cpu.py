@@ -95,12 +95,12 @@ def test_workspace_bytes_and_strerror(lib):
     for L in (4, 64, 100, 1024, 16384):
         wb = lib.sw_workspace_bytes(L, 2)
         ntx, nty = -(-L // 128), -(-L // 32)
-        # cluster sizes + the two int32 edge arrays + the draw cache (1 byte per 4 sites of every strip)
-        need = 4 * L * L + 2 * 4 * (ntx + nty) * L + ntx * nty * 1024
+        # cluster sizes + the two int32 edge arrays (the draw cache is not part of the default build: nothing reserved for it)
+        need = 4 * L * L + 2 * 4 * (ntx + nty) * L
         assert need <= wb < need + 65536 + 4096 * 16 + 16384    # + the (sat, minus) ring of sw_series_read, accumulators
     assert lib.sw_workspace_bytes(32768, 2) > 0 and lib.sw_workspace_bytes(32768, 3) == 0   # q > 2: L <= 16384
     assert lib.sw_strerror(0) == b"ok"
-    for code in (-1, -2, -3, -4, -99):
+    for code in (-1, -2, -3, -4, -5, -99):
         assert len(lib.sw_strerror(code)) > 0
 
 

@@ -72,3 +72,11 @@ def test_reference_arm_nonzero_rank_is_silent():
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2",
                         "--L", "128", "--steps", "1"], capture_output=True, text=True, timeout=120, env=env)
     assert r.returncode == 0 and r.stdout.strip() == ""
+
+
+def test_bench_percolation_thresholds_are_the_stored_golden_integers():
+    """bench.py passes BASELINE.json configs[3]'s bond thresholds to sw_set_threshold as integers; they are the values of
+    tests/golden/thresholds.txt (pinned there to the closed forms), not something the bench computes."""
+    from conftest import read_golden
+    g = read_golden("thresholds.txt")
+    assert bench.PERC_THRESHOLD == {0.3: int(g["perc_0.3"]), 0.5: int(g["perc_0.5"]), 0.7: int(g["perc_0.7"])}

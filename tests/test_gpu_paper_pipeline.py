@@ -39,9 +39,10 @@ def paper_case(L, codes, methods=(0, 1), Bs=(8, 16, 32)):
             assert lat.observables(spins=False, clusters=False)["n_clusters"] == nc
             assert 1 <= st["selflabel_passes_max"] <= B * B
             if method == 0:
-                assert st["relax_iterations"] >= 1 and st["sewing_levels"] == 0
+                assert st["relax_iterations"] >= 1 and st["sewing_levels"] == 0 and st["ms_wrap"] == 0.0
             else:
                 assert st["sewing_levels"] == int(math.log2(L // B)) and st["relax_iterations"] == 0
+                assert 0.0 < st["ms_wrap"] <= st["ms_consolidate"]          # the wrap-around step is timed on its own
     lat.close()
 
 
