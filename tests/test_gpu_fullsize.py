@@ -143,7 +143,7 @@ def test_config3_L16384_off_critical_vs_oracle(beta):
 def test_L16384_labelling_repeats_bit_for_bit(what):
     """compute-sanitizer is closed on this GPU pool, so races are hunted by repetition at the size and contention of
     the bench: the same packed bonds are labelled 30 times; every result must equal the first (the canonical labelling
-    is unique, reading 7) and the first must satisfy the bond-end check."""
+    is unique, reading 7) and the first must equal the oracle's labelling of the same bonds."""
     L = 16384
     lat = binding.Lattice(L, 2, 0.5, 3, with_bonds=True)
     if what.startswith("p="):
@@ -156,6 +156,9 @@ def test_L16384_labelling_repeats_bit_for_bit(what):
     first = torch.empty(L * L, dtype=torch.int32, device="cuda")
     lat.label(lat.bonds, first)
     check_label_properties(L, first, lat.bonds)
+    want, _ = oracle.label(L, oracle.unpack_bonds(lat.bonds.cpu().numpy(), L * L))   # the first against the oracle, once
+    assert np.array_equal(first.cpu().numpy(), want), what
+    del want
     out = torch.empty_like(first)
     for rep in range(30):
         out.fill_(-7)
@@ -202,8 +205,8 @@ def test_L32768_largest_lattice_properties():
 
 
 def test_config4_L16384_percolation_labels_and_densities():
-    """BASELINE.json configs[3]: i.i.d. bonds at p in {0.3, 0.5, 0.7}; p=0.5 labels against the oracle bit for bit, all
-    three against the invariants; cluster densities against the pins of SURVEY.md 8(c) (square-lattice bond percolation:
+    """BASELINE.json configs[3]: i.i.d. bonds at p in {0.3, 0.5, 0.7}; bonds and labels of all three against the oracle
+    bit for bit and against the invariants; cluster densities against the pins of SURVEY.md 8(c) (square-lattice bond percolation:
     n_c(1/2) = (3 sqrt 3 - 5)/2 per site; Euler duality n_c(0.3) - n_c(0.7) = 1 - 2*0.3)."""
     L, N = 16384, 16384 * 16384
     lat = binding.Lattice(L, 2, 0.1, 1, with_bonds=True)
@@ -218,14 +221,14 @@ def test_config4_L16384_percolation_labels_and_densities():
         st = lat.cluster_stats()
         assert st["n_clusters"] == nroots and sum(st["hist32"]) == nroots
         dens[p] = nroots / N
-        if p == 0.5:
-            codes = oracle.unpack_bonds(lat.bonds.cpu().numpy(), N)
-            want_codes, _ = oracle.bonds(L, oracle.threshold_from_p(p), 1, 0, oracle.init_spins(L, 2, 1, 0))
-            assert np.array_equal(codes, want_codes)
-            del want_codes
-            want, nc = oracle.label(L, codes)
-            assert nc == nroots and np.array_equal(lat.labels_host(), want)
-            del want, codes
+        # every p against the oracle bit for bit (the invariants above cannot see two clusters sharing one label)
+        codes = oracle.unpack_bonds(lat.bonds.cpu().numpy(), N)
+        want_codes, _ = oracle.bonds(L, oracle.threshold_from_p(p), 1, 0, oracle.init_spins(L, 2, 1, 0))
+        assert np.array_equal(codes, want_codes), p
+        del want_codes
+        want, nc = oracle.label(L, codes)
+        assert nc == nroots and np.array_equal(lat.labels_host(), want), p
+        del want, codes
     sigma = math.sqrt(0.15 / N)                                       # per-sample sigma of clusters/N
     assert abs(dens[0.5] - ((3 * math.sqrt(3) - 5) / 2 + 0.8835 / N)) < 5 * sigma
     assert abs((dens[0.3] - dens[0.7]) - 0.4) < 5 * math.sqrt(2) * sigma
