@@ -552,6 +552,23 @@ def run_ours(args):
     barrier()
     e2e_ms, e2e_units = aggregate_over_ranks(ev0.elapsed_time(ev1), float(N) * e2e_steps, dist if world > 1 else None)
     e2e_ns = e2e_ms * 1e6 / e2e_units
+    # the same call with the 4N bytes of labels copied back as well (rank 0, two steps: a second figure, not the e2e value)
+    e2e_labels = None
+    if rank == 0 and not args.no_e2e_labels:
+        h_lab = torch.empty(N, dtype=torch.int32).pin_memory()
+        lat.sweep_host(h_in, 1, h_out, h_lab, obs_flags=binding.OBS_SPINS)
+        torch.cuda.synchronize(device)
+        ev0.record(stream)
+        for _ in range(2):
+            lat.sweep_host(h_in, 1, h_out, h_lab, obs_flags=binding.OBS_SPINS)
+            h_in, h_out = h_out, h_in
+        ev1.record(stream)
+        torch.cuda.synchronize(device)
+        ms_lab = ev0.elapsed_time(ev1) / 2
+        e2e_labels = {"ms_per_step": ms_lab, "ns_per_spin_update": ms_lab * 1e6 / N, "h2d_bytes_per_step": N,
+                      "d2h_bytes_per_step": N + 4 * N + 128, "steps": 2,
+                      "what": "as e2e, plus the int32 labels of the sweep copied to pinned host memory"}
+        del h_lab
 
     if rank != 0:
         lat.close()
@@ -627,7 +644,8 @@ def run_ours(args):
         "e2e": {"value": e2e_ns, "unit": "ns", "h2d_bytes_per_step": N, "d2h_bytes_per_step": N + 128,
                 "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps,
                 "what": "sw_sweep_host_ex(SW_OBS_SPINS): pinned host spins -> device, one sweep, spins + sw_obs (energy, magnetisation, "
-                        "state counts, cluster and bond counts; no cluster-size pass) back to the host"},
+                        "state counts, cluster and bond counts; no cluster-size pass) back to the host; the labels stay on the device",
+                "with_labels_copied_back": e2e_labels},
         "gpu_launches": launches,
         "roofline": roofline,
         "cpu_baseline": cpu,
@@ -655,6 +673,7 @@ def main(argv=None):
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e-labels", action="store_true", help="skip the second end-to-end figure (labels copied back too; 1 GiB pinned)")
     ap.add_argument("--no-labelling", action="store_true")
     ap.add_argument("--bands", action="store_true", help="with --gpus N under torchrun: one lattice in N row bands (strong scaling) instead of N replicas")
     ap.add_argument("--bands-one-gpu", type=int, default=0, metavar="G", help="time the G-band algorithm band after band on one GPU next to sw_sweep")
