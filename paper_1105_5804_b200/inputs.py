@@ -66,3 +66,29 @@ def spiral_codes(L: int) -> np.ndarray:
     codes[0, : L - 1] |= 1
     codes[: L - 1, :] |= 2
     return codes.reshape(-1)
+
+
+def blob_image(L: int, levels: int, seed: int, smooth: int = 3) -> np.ndarray:
+    """uint8[L, L] synthetic grey-level image: seeded uniform noise, box-smoothed `smooth` times (3 x 3, no wrap), quantised to
+    `levels` grey levels of equal population -- blobs of all sizes with ragged outlines, the structure of a segmentation input
+    ("image segmentation").  Stands in for no dataset."""
+    rng = np.random.default_rng(seed)
+    a = rng.random((L, L))
+    for _ in range(smooth):
+        b = np.pad(a, 1, mode="edge")
+        a = sum(b[1 + dy:1 + dy + L, 1 + dx:1 + dx + L] for dy in (-1, 0, 1) for dx in (-1, 0, 1)) / 9.0
+    ranks = a.reshape(-1).argsort(kind="stable").argsort(kind="stable")
+    return (ranks * levels // (L * L)).astype(np.uint8).reshape(L, L)
+
+
+def image_bond_codes(img: np.ndarray) -> np.ndarray:
+    """uint8[N] bond codes (the boundary's format: bit0 east, bit1 north) of the pixel-adjacency graph of an L x L image with
+    4-connectivity: a bond joins two neighbouring pixels of equal value.  Row 0 of the array is lattice row y = 0.  An image
+    has no periodic boundary: the east bonds of the last column and the north bonds of the last row stay open.  This is input
+    preparation for sw_label (a graph handed to the labeller), not part of the method."""
+    L = img.shape[0]
+    assert img.shape == (L, L)
+    codes = np.zeros((L, L), dtype=np.uint8)
+    codes[:, : L - 1] |= (img[:, : L - 1] == img[:, 1:]).astype(np.uint8)
+    codes[: L - 1, :] |= ((img[: L - 1, :] == img[1:, :]).astype(np.uint8) << 1)
+    return codes.reshape(-1)

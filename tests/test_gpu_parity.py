@@ -67,6 +67,13 @@ def label_case(L, codes):
     lat.close()
 
 
+@pytest.mark.parametrize("L,levels,seed", [(64, 2, 1), (132, 3, 2), (516, 4, 3), (1024, 2, 4), (1024, 6, 5)])
+def test_label_image_segments(L, levels, seed):
+    """A generic CCL input ("image segmentation"): sw_label on the 4-connected equal-value pixel graph of a
+    synthetic grey-level image (no periodic bonds, blobs of all sizes) against the oracle, with cluster statistics."""
+    label_case(L, inputs.image_bond_codes(inputs.blob_image(L, levels, seed)))
+
+
 @pytest.mark.parametrize("L", [4, 8, 12, 64, 100, 128, 132, 192, 256, 260, 516, 1024])
 @pytest.mark.parametrize("p", [0.3, 0.5, 0.7])
 def test_label_random_bonds(L, p):

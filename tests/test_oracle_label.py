@@ -218,3 +218,27 @@ def test_percolation_cluster_density_and_duality():
     sigma = math.sqrt(0.15 / N / 3)
     assert abs(dens[0.5] - ((3 * math.sqrt(3) - 5) / 2 + 0.8835 / N)) < 5 * sigma
     assert abs((dens[0.3] - dens[0.7]) - 0.4) < 5 * math.sqrt(2) * sigma
+
+
+def test_label_of_an_image_adjacency_graph_matches_ndimage_segments():
+    """Generic CCL input ("image segmentation"): the oracle's labelling of the 4-connected equal-value
+    pixel graph of a synthetic image against scipy.ndimage.label run grey level by grey level (an independent labeller with
+    its own numbering: compared as partitions, and the oracle's label must be the smallest pixel index of its segment)."""
+    from scipy import ndimage
+    for L, levels, seed in ((64, 2, 1), (100, 3, 2), (132, 5, 3)):
+        img = inputs.blob_image(L, levels, seed)
+        assert len(np.unique(img)) == levels
+        codes = inputs.image_bond_codes(img)
+        assert not (codes.reshape(L, L)[:, L - 1] & 1).any() and not (codes.reshape(L, L)[L - 1, :] & 2).any()   # no wrap
+        lab, nc = oracle.label(L, codes)
+        seg = np.zeros((L, L), dtype=np.int64)
+        total = 0
+        for v in range(levels):
+            s, n = ndimage.label(img == v)                      # default structure: 4-connectivity
+            seg[s > 0] = s[s > 0] + total
+            total += n
+        assert nc == total
+        seg = seg.reshape(-1)
+        first = np.full(total + 1, L * L, dtype=np.int64)
+        np.minimum.at(first, seg, np.arange(L * L))
+        assert np.array_equal(lab, first[seg].astype(np.int32))
