@@ -9,7 +9,10 @@ namespace swb {
 // Strip of the one-level decomposition ("tiles of B_x x B_y spins", P:84 B_x >> B_y for coalescing).
 // k_scan: one WARP labels a TW x TH strip, lane -> 4 consecutive columns (one 32-bit word of int8 spins, one 128-bit
 // vector of int32 labels), rows in sequence.  k_final: one CTA of FIN_THREADS threads per strip.
-constexpr int TW_LOG = 7, TH_LOG = 5;
+#ifndef SWB_TH_LOG
+#define SWB_TH_LOG 5
+#endif
+constexpr int TW_LOG = 7, TH_LOG = SWB_TH_LOG;           // (TH = 16 needs SWB_FIN_THREADS = 128: k_final's warps own 4 rows each)
 constexpr int TW = 1 << TW_LOG;
 constexpr int TH = 1 << TH_LOG;
 #ifndef SWB_SCAN_WARPS

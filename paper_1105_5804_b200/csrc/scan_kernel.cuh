@@ -376,13 +376,16 @@ struct ScanSmem {
 // FULLW: L is a multiple of TW, every strip has all 32 lanes (no ragged right edge; the predicates fold away).
 enum { SRC_PHILOX = 0, SRC_BONDS = 1, SRC_DRAWS = 2 };
 template <int SRC, bool ISING, bool FULLW, bool BAND = false>    // BAND: strip row = blockIdx.y + ty0 (see k_final)
-__global__ void __launch_bounds__(SCAN_THREADS, 24 / SCAN_WARPS)    // 24 warps per SM (shared memory): up to 85 registers
+#ifndef SWB_SCAN_RES_WARPS
+#define SWB_SCAN_RES_WARPS 24
+#endif
+__global__ void __launch_bounds__(SCAN_THREADS, SWB_SCAN_RES_WARPS / SCAN_WARPS)    // 24 warps per SM (shared memory): up to 85 registers
 k_scan(const Params p, const uint32_t* __restrict__ spins_w, const uint8_t* __restrict__ bonds_in,
        const uint32_t* __restrict__ draws, int* prov, int* __restrict__ edgeA, int* __restrict__ edgeB,
        Acc* __restrict__ acc)
 {
     constexpr bool FROM_BONDS = SRC == SRC_BONDS;
-    extern __shared__ __align__(16) unsigned char s_raw[];   // ScanSmem: more than the 48 KB a static allocation may have
+    extern __shared__ __align__(16) unsigned char s_raw[];   // ScanSmem: 37.9 KB with SCAN_WARPS = 4; dynamic because a SCAN_WARPS = 8 build exceeds the 48 KB of a static allocation
     ScanSmem& sm = *reinterpret_cast<ScanSmem*>(s_raw);
     uint4* const s_la = sm.la;
     uint4* const s_lb = sm.lb;
