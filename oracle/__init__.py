@@ -103,6 +103,11 @@ def lib():
         L.orc_wolff_step.restype = C.c_int64
         L.orc_wolff_chain.argtypes = [C.c_int32, C.c_uint32, C.c_uint64, C.c_uint64, C.c_int64, p8, p64]
         L.orc_wolff_chain.restype = C.c_int
+        L.orc_fewcluster_step.argtypes = [C.c_int32, C.c_int32, C.c_uint32, C.c_uint64, C.c_uint64, C.c_int32, C.c_uint32, p8,
+                                          C.POINTER(C.c_int32), p64]
+        L.orc_fewcluster_step.restype = C.c_int64
+        L.orc_fewcluster_chain.argtypes = [C.c_int32, C.c_uint32, C.c_uint64, C.c_uint64, C.c_int64, C.c_int32, C.c_uint32, p8, p64]
+        L.orc_fewcluster_chain.restype = C.c_int
         L.orc_fnv1a64.argtypes = [pu8, C.c_int64]
         L.orc_fnv1a64.restype = C.c_uint64
         # simple cubic lattice
@@ -252,6 +257,26 @@ def wolff_chain(L: int, T: int, seed: int, t0: int, n: int, spins: np.ndarray) -
     assert spins.dtype == np.int8 and spins.size == L * L and spins.flags.c_contiguous
     series = np.zeros((n, 3), dtype=np.int64)
     if lib().orc_wolff_chain(L, T, seed, t0, n, _p(spins, C.c_int8), _p(series, C.c_int64)) != 0:
+        raise MemoryError
+    return series
+
+
+def fewcluster_step(L: int, T: int, seed: int, t: int, n_seeds: int, T_flip: int, spins: np.ndarray):
+    """One few-cluster step in place (q=2, reading 21). -> (flipped sites, flipped clusters, labels)"""
+    assert spins.dtype == np.int8 and spins.size == L * L and spins.flags.c_contiguous
+    labels = np.empty(L * L, dtype=np.int32)
+    nfc = C.c_int64(0)
+    f = lib().orc_fewcluster_step(L, 2, T, seed, t, n_seeds, T_flip, _p(spins, C.c_int8), _p(labels, C.c_int32), C.byref(nfc))
+    if f < 0:
+        raise MemoryError
+    return int(f), int(nfc.value), labels
+
+
+def fewcluster_chain(L: int, T: int, seed: int, t0: int, n: int, n_seeds: int, T_flip: int, spins: np.ndarray) -> np.ndarray:
+    """n few-cluster steps in place; -> int64[n,3] = (E, M, flipped sites) after every step."""
+    assert spins.dtype == np.int8 and spins.size == L * L and spins.flags.c_contiguous
+    series = np.zeros((n, 3), dtype=np.int64)
+    if lib().orc_fewcluster_chain(L, T, seed, t0, n, n_seeds, T_flip, _p(spins, C.c_int8), _p(series, C.c_int64)) != 0:
         raise MemoryError
     return series
 

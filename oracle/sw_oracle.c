@@ -392,6 +392,73 @@ uint64_t orc_fnv1a64(const uint8_t *p, int64_t n)
     return h;
 }
 
+/* ---- S:8f row 1, second half: the few-cluster variant.  The paper grows clusters from
+ * several seed sites at once and gives every cluster "a flipping probability p_flip < 1"; it states that this is
+ * "logically identical to performing the full SW decomposition and then selecting [...] points on the lattice,
+ * followed by flipping all distinct clusters these points belong to".  That statement is what is written out here
+ * (reading 21 fixes what the paper leaves open -- the draws):
+ *   bonds and labels of step t as in a sweep (S:8c.3-5, on the pre-step spins);
+ *   seed sites i_k = (PHILOX(seed; k, t, WSEED)[0] * N) >> 32, k = 0 .. n_seeds-1 (k = 0 is the Wolff seed, S:8c.9);
+ *   a cluster is selected iff it holds at least one seed site (a cluster hit twice is one cluster);
+ *   a selected cluster with root r is flipped (s -> -s on all its sites) iff PHILOX(seed; r, t, FLIP)[1] < T_flip
+ *   (word 1: word 0 is the state draw of a sweep), T_flip = floor(p_flip 2^32), so p_flip < 1 always.
+ * Returns the number of flipped sites; *n_flipped_clusters the number of flipped clusters; labels_out (N, or
+ * NULL) the canonical labels of the decomposition.  q must be 2 (as for Wolff).  t += 1 is the caller's.
+ * Pins (tests/test_oracle_physics.py): a numpy restatement from the pinned bonds / labels / Philox; one seed at
+ * T_flip = 2^32 - 1 equals orc_wolff_step (ties the seed keying to the golden Wolff vectors); exact <E>, <|m|> of
+ * the 4 x 4 Ising model for a chain with 3 seeds and p_flip = 0.7 (detailed balance holds cluster by cluster). */
+int64_t orc_fewcluster_step(int32_t L, int32_t q, uint32_t T, uint64_t seed, uint64_t t, int32_t n_seeds,
+                            uint32_t T_flip, int8_t *spins, int32_t *labels_out, int64_t *n_flipped_clusters)
+{
+    int64_t N = (int64_t)L * L, flipped = 0, nfc = 0;
+    if (q != 2 || n_seeds < 0) return -1;
+    uint8_t *codes = (uint8_t *)malloc((size_t)N);
+    int32_t *labels = (int32_t *)malloc((size_t)N * sizeof(int32_t));
+    uint8_t *selected = (uint8_t *)calloc((size_t)N, 1);          /* selected[r]: root r holds a seed site */
+    if (!codes || !labels || !selected) { free(codes); free(labels); free(selected); return -1; }
+    orc_bonds(L, T, seed, t, spins, codes);
+    orc_label(L, codes, labels);
+    for (int32_t k = 0; k < n_seeds; ++k) {
+        uint32_t w[4];
+        draw(seed, (uint32_t)k, t, DOM_WSEED, w);
+        int64_t ik = (int64_t)(((uint64_t)w[0] * (uint64_t)N) >> 32);
+        selected[labels[ik]] = 1;
+    }
+    for (int64_t i = 0; i < N; ++i) {
+        int32_t r = labels[i];
+        if (!selected[r]) continue;
+        uint32_t w[4];
+        draw(seed, (uint32_t)r, t, DOM_FLIP, w);
+        if (w[1] < T_flip) {
+            spins[i] = (int8_t)(-spins[i]);
+            ++flipped;
+            if (i == r) ++nfc;
+        }
+    }
+    if (labels_out) memcpy(labels_out, labels, (size_t)N * sizeof(int32_t));
+    if (n_flipped_clusters) *n_flipped_clusters = nfc;
+    free(codes); free(labels); free(selected);
+    return flipped;
+}
+
+/* chain of n few-cluster steps; series[3*s + 0..2] = energy, magnetisation, flipped sites */
+int orc_fewcluster_chain(int32_t L, uint32_t T, uint64_t seed, uint64_t t0, int64_t n, int32_t n_seeds,
+                         uint32_t T_flip, int8_t *spins, int64_t *series)
+{
+    for (int64_t s = 0; s < n; ++s) {
+        int64_t f = orc_fewcluster_step(L, 2, T, seed, t0 + (uint64_t)s, n_seeds, T_flip, spins, NULL, NULL);
+        if (f < 0) return -1;
+        if (series) {
+            orc_obs o;
+            orc_observables(L, 2, spins, &o);
+            series[3 * s + 0] = o.energy;
+            series[3 * s + 1] = o.magnetisation;
+            series[3 * s + 2] = f;
+        }
+    }
+    return 0;
+}
+
 /* ==================================================================================
  * Simple cubic lattice ("hypercubic lattices", P:154
  * "three out of six neighbours" are looked after by every site in 3D).  The same

@@ -196,6 +196,65 @@ def test_wolff_equals_label_then_flip_one_cluster():
         assert 0 <= i0 < L * L
 
 
+# ---------------------------------------------------------------- few-cluster variant -------------
+def test_fewcluster_equals_decompose_select_flip():
+    """The paper's own statement of the variant: full SW decomposition, select points, flip the distinct clusters
+    they belong to -- each with probability p_flip.  Restated in numpy from the pinned pieces (bonds, labels, the KAT-pinned
+    Philox) with the keying of DESIGN.md reading 21: seeds (k, t, WSEED)[0], flip decision (root, t, FLIP)[1] < T_flip."""
+    L, seed = 24, 77 + (1 << 35)
+    N = L * L
+    T = oracle.threshold(2, BETA_C)
+    key = [seed & 0xFFFFFFFF, seed >> 32]
+    s = oracle.init_spins(L, 2, seed, 1)
+    seen_partial = False
+    for t, n_seeds, T_flip in [(0, 1, 0xFFFFFFFF), (1, 5, 0x80000000), (2, 40, 0xB3333333), ((7 << 32) + 3, 17, 0x40000000),
+                               (4, 9, 0), (5, 0, 0xFFFFFFFF)]:
+        before = s.copy()
+        codes, _ = oracle.bonds(L, T, seed, t, before)
+        lab, _ = oracle.label(L, codes)
+        tl, th = t & 0xFFFFFFFF, t >> 32
+        roots = {int(lab[(int(oracle.philox([k, tl, th, 3], key)[0]) * N) >> 32]) for k in range(n_seeds)}
+        flip_roots = [r for r in sorted(roots) if int(oracle.philox([r, tl, th, 2], key)[1]) < T_flip]
+        want = before.copy()
+        m = np.isin(lab, flip_roots)
+        want[m] = -want[m]
+        f, nfc, lab_o = oracle.fewcluster_step(L, T, seed, t, n_seeds, T_flip, s)
+        assert np.array_equal(lab_o, lab) and np.array_equal(s, want)
+        assert f == int(m.sum()) and nfc == len(flip_roots)
+        seen_partial = seen_partial or (0 < len(flip_roots) < len(roots))
+    assert seen_partial                                          # some selected cluster was NOT flipped: p_flip < 1 is exercised
+
+
+def test_fewcluster_with_one_seed_and_pflip_one_is_the_wolff_step():
+    """n_seeds = 1, T_flip = 2^32 - 1: the seed (0, t, WSEED)[0] is the Wolff seed and its cluster is flipped (unless the one
+    draw equals 2^32 - 1): the same configuration as orc_wolff_step, whose keying the survey's golden vectors pin."""
+    L, seed = 32, 1234
+    T = oracle.threshold(2, BETA_C)
+    a = oracle.init_spins(L, 2, seed, 1)
+    b = a.copy()
+    for t in range(60):
+        sz, i0, root = oracle.wolff_step(L, T, seed, t, a)
+        f, nfc, lab = oracle.fewcluster_step(L, T, seed, t, 1, 0xFFFFFFFF, b)
+        assert (f, nfc) == (sz, 1) and lab[i0] == root and np.array_equal(a, b), t
+
+
+@pytest.mark.slow
+def test_fewcluster_4x4_reproduces_exact_enumeration():
+    """Flipping any subset of FK clusters chosen independently of the spins, each with a probability that depends on the bond
+    configuration only, keeps the Boltzmann weight stationary: <E> and <|m|> of the 4 x 4 model, 3 seeds, p_flip = 0.7."""
+    L, N = 4, 16
+    E, M = enumerate_ising(L)
+    e_x, am_x, m2_x, _ = boltzmann_averages(E, M, BETA_C, N)
+    T = oracle.threshold(2, BETA_C)
+    s = oracle.init_spins(L, 2, 5, 1)
+    ser = oracle.fewcluster_chain(L, T, 5, 0, 1_500_000, 3, oracle.threshold_from_p(0.7), s)[1000:]
+    e, m = ser[:, 0] / N, ser[:, 1] / N
+    assert abs(e.mean() - e_x) < 4.5 * blocked_error(e)
+    assert abs(np.abs(m).mean() - am_x) < 4.5 * blocked_error(np.abs(m))
+    assert abs((m * m).mean() - m2_x) < 4.5 * blocked_error(m * m)
+    assert 0 < ser[:, 2].mean() < N
+
+
 def test_wolff_seed_sites_are_uniform():
     L, N = 16, 256
     T = oracle.threshold(2, 0.2)
