@@ -196,6 +196,19 @@ int sw_label_paper(sw_handle* h, int method, int B, const uint8_t* d_bonds_in, i
  * step -- in that case the call synchronises `stream` before returning. */
 int wolff_step(sw_handle* h, int64_t n, int64_t* h_sizes, void* stream);
 
+/* n steps of the FEW-CLUSTER variant (S:8f row 1), q = 2 on the square lattice only (SW_EINVAL otherwise); t += n.
+ * The paper grows clusters from many seed sites at once and flips each with "a flipping probability p_flip < 1", and states
+ * that this is "logically identical to performing the full SW decomposition and then selecting [...] points on the lattice,
+ * followed by flipping all distinct clusters these points belong to"; that is what a step at counter t does (DESIGN.md
+ * reading 21 fixes the draws): bonds and canonical labels as in sw_sweep; seed sites i_k = (PHILOX(seed; k, t, WSEED)[0] * N)
+ * >> 32, k < n_seeds (k = 0 is wolff_step's seed); every cluster that holds a seed site is selected once; a selected cluster
+ * with root r has all its spins negated iff PHILOX(seed; r, t, FLIP)[1] < T_flip, i.e. with probability T_flip / 2^32 < 1.
+ * 0 <= n_seeds <= 65536, and the next power of two >= 2 n_seeds must not exceed N (the table of selected roots uses the
+ * cluster-size scratch of the workspace).  d_labels holds the canonical labels of the last step's decomposition; the energy
+ * series and the cluster part of sw_obs are maintained as by sw_sweep.  h_flipped: NULL, or a HOST array of n int64 that
+ * receives the number of flipped sites of every step -- then the call synchronises `stream`. */
+int sw_fewcluster_step(sw_handle* h, int64_t n, int32_t n_seeds, uint32_t T_flip, int64_t* h_flipped, void* stream);
+
 /* Frontier growth for wolff_step (P:355 option (b); S:8f.1).  max_levels = 0 (default): every step decomposes the whole
  * lattice and flips one cluster.  max_levels > 0: a step first grows the cluster from the seed site level by level --
  * the bond draws are pure functions of (seed, t, site, direction), so it is the same cluster, and only the bonds that

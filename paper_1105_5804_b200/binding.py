@@ -24,7 +24,7 @@ SYMBOLS = [
     "sw_cluster_stats", "wolff_step", "sw_observables", "sw_observables_ex", "sw_series_read", "sw_wolff_frontier", "sw_sweep_host", "sw_sweep_host_ex", "sw_launch_count", "sw_strerror",
     "sw_last_cuda_error", "sw_profile_enable", "sw_profile_read", "sw_create3d", "sw_workspace_bytes3d", "sw_label_paper",
     "sw_set_band", "sw_band_layout", "sw_sweep_band_begin", "sw_sweep_band_end", "sw_band_counters",
-    "sw_cluster_stats_static",
+    "sw_cluster_stats_static", "sw_fewcluster_step",
 ]
 
 
@@ -97,6 +97,7 @@ def lib():
     L.sw_sweep_band_end.argtypes = [vp, vp]
     L.sw_band_counters.argtypes = [vp, C.POINTER(i64), vp]
     L.wolff_step.argtypes = [vp, i64, C.POINTER(i64), vp]
+    L.sw_fewcluster_step.argtypes = [vp, i64, i32, u32, C.POINTER(i64), vp]
     L.sw_observables.argtypes = [vp, C.POINTER(sw_obs), vp]
     L.sw_observables_ex.argtypes = [vp, C.POINTER(sw_obs), C.c_int, vp]
     L.sw_wolff_frontier.argtypes = [vp, C.c_int]
@@ -267,6 +268,15 @@ class Lattice:
             self._check(self._lib.wolff_step(self._h, n, sizes, self._stream()))
             return list(sizes)
         self._check(self._lib.wolff_step(self._h, n, None, self._stream()))
+        return None
+
+    def fewcluster_step(self, n: int, n_seeds: int, T_flip: int, want_counts: bool = True):
+        """n few-cluster steps (sw_fewcluster_step) -> list of flipped sites per step, or None"""
+        if want_counts:
+            out = (C.c_int64 * n)()
+            self._check(self._lib.sw_fewcluster_step(self._h, n, n_seeds, T_flip, out, self._stream()))
+            return list(out)
+        self._check(self._lib.sw_fewcluster_step(self._h, n, n_seeds, T_flip, None, self._stream()))
         return None
 
     def wolff_frontier(self, max_levels: int):

@@ -62,6 +62,8 @@ struct Params {
     int32_t  n3x, n3y, n3z;   // simple cubic lattice: number of tiles per direction (cubic_kernels.cuh), else 0
     int32_t  ty0, nband;      // row band of a multi-GPU run (band_kernels.cuh): first strip row and number of strip rows this
                               // handle works on; 0 and nty for the whole lattice
+    uint32_t T_flip;          // few-cluster step (k_final<MODE_FEW>): a selected cluster is flipped iff its draw is < T_flip
+    int32_t  few_mask;        // ... and the table of selected roots has few_mask + 1 slots (a power of two)
 };
 
 // Philox4x32-10 (Salmon et al., SC'11).  c1,c2,c3 are warp-uniform in every use here (step counter and domain).

@@ -231,7 +231,51 @@ k_seam(const Params p, const int* __restrict__ edgeA, const int* __restrict__ ed
 }
 
 // ------------------------------------------------------------------------------------------------ k_final
-enum { MODE_SW = 0, MODE_WOLFF = 1, MODE_LABEL = 2 };
+enum { MODE_SW = 0, MODE_WOLFF = 1, MODE_LABEL = 2, MODE_FEW = 3 };
+
+// ---- few-cluster step (S:8f row 1; reading 21): "full SW decomposition, select points, flip the distinct
+// clusters these points belong to", each with probability p_flip.  k_few_seeds (one CTA, after k_seam) resolves the seed sites
+// i_k = (PHILOX(seed; k, t, WSEED)[0] N) >> 32 to the roots of their global trees and enters them into a small open-addressing
+// table in the workspace (-1 = empty; at least twice as many slots as seeds); k_final<MODE_FEW> looks every strip-local root's
+// global root up in it and, for a selected one, draws PHILOX(seed; r, t, FLIP)[1] < T_flip.
+__device__ __forceinline__ uint32_t few_slot(int root, int mask) { return ((uint32_t)root * 0x9E3779B1u >> 7) & (uint32_t)mask; }
+
+__global__ void __launch_bounds__(256)
+k_few_seeds(const Params p, const int* labels, int* __restrict__ table, int n_seeds)
+{
+    const int L = p.L;
+    for (int i = threadIdx.x; i <= p.few_mask; i += blockDim.x) table[i] = -1;
+    __syncthreads();
+    for (int k = threadIdx.x; k < n_seeds; k += blockDim.x) {
+        uint32_t w0, w1, w2, w3;
+        philox4x32_10(p, (uint32_t)k, p.t_lo, p.t_hi, DOM_WSEED, w0, w1, w2, w3);
+        const int i0 = (int)__umulhi(w0, (uint32_t)p.N);
+        const int iy = i0 / L, ix = i0 - iy * L;
+        const int b0 = (iy / TH * TH) * L + (ix / TW * TW);
+        const int r = gfind(labels, strip_root(labels, L, i0, b0));
+        uint32_t slot = few_slot(r, p.few_mask);
+        while (true) {                                   // the table is never full: slots >= 2 n_seeds
+            const int old = atomicCAS(&table[slot], -1, r);
+            if (old == -1 || old == r) break;
+            slot = (slot + 1) & (uint32_t)p.few_mask;
+        }
+    }
+}
+
+// is `root` a selected root, and does its draw flip it?  (The Philox call runs for selected roots only: few.)
+__device__ __forceinline__ uint32_t few_flips(const Params& p, const int* __restrict__ table, int root)
+{
+    uint32_t slot = few_slot(root, p.few_mask);
+    while (true) {
+        const int e = __ldg(table + slot);
+        if (e == root) break;
+        if (e == -1) return 0u;
+        slot = (slot + 1) & (uint32_t)p.few_mask;
+    }
+    uint32_t w0, w1, w2, w3;
+    philox4x32_10(p, (uint32_t)root, p.t_lo, p.t_hi, DOM_FLIP, w0, w1, w2, w3);
+    return w1 < p.T_flip ? 1u : 0u;
+}
 
 __device__ __forceinline__ uint32_t flip_state(const Params& p, int root)
 {
@@ -262,6 +306,8 @@ __device__ __forceinline__ int lds_s32(uint32_t saddr)
 //   MODE_SW    : s_i = state drawn for the root (assign, P:55 step 3)
 //   MODE_WOLFF : s_i = -s_i iff root(i) == root(seed site i0); adds |C| to *wolff_size
 //   MODE_LABEL : labels only
+//   MODE_FEW   : s_i = -s_i iff root(i) is a selected root whose draw is < T_flip (few-cluster step; the table of selected
+//                roots comes in through the `draws` argument); adds the number of flipped sites to *wolff_size
 // (1) every warp copies its rows of entries to shared memory and lists the strip-local roots among them; (2) it resolves
 // each of them to the root of its global tree (a chase over entries >= 0 of other strips, which concurrently running CTAs
 // may already have overwritten with final labels -- those are roots of the same tree, so the chase still ends at the
@@ -386,7 +432,8 @@ k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __rest
         __syncwarp(__activemask());
         nroots += (v == g);
         // final label and, above bit p.sbit, the new state of the cluster (labels are < 2^sbit)
-        sm.S[l] = MODE == MODE_SW ? (int)((uint32_t)v | (flip_state(p, v) << p.sbit)) : v;
+        if (MODE == MODE_FEW) sm.S[l] = (int)((uint32_t)v | (few_flips(p, reinterpret_cast<const int*>(draws), v) << p.sbit));
+        else sm.S[l] = MODE == MODE_SW ? (int)((uint32_t)v | (flip_state(p, v) << p.sbit)) : v;
     }
     nroots = __reduce_add_sync(FULLM, nroots);
     __syncthreads();
@@ -427,6 +474,16 @@ k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __rest
                 if (Q2) word = 0x01010101u | (word * 0xFEu);   // k=0 -> +1 (0x01), k=1 -> -1 (0xFF)
                 *srow = word;
                 *reinterpret_cast<int4*>(lrow) = make_int4(ww[0] & lmask, ww[1] & lmask, ww[2] & lmask, ww[3] & lmask);
+            } else if (MODE == MODE_FEW) {
+                // the 4 top bytes hold the flip bits above bit sbit - 24: bytes 0 / 1 -> negate the spins of the 1-bytes
+                const uint32_t t = __byte_perm(__byte_perm(ww[0], ww[1], 0x0073), __byte_perm(ww[2], ww[3], 0x0073), 0x5410);
+                const uint32_t word = (t >> sshift) & smask & 0x01010101u;
+                if (word) {
+                    const uint32_t m = word * 0xFFu, old = *srow;
+                    *srow = __vneg4(old & m) | (old & ~m);
+                    nflip += __popc(word);
+                }
+                *reinterpret_cast<int4*>(lrow) = make_int4(ww[0] & lmask, ww[1] & lmask, ww[2] & lmask, ww[3] & lmask);
             } else {
                 *reinterpret_cast<int4*>(lrow) = make_int4(ww[0], ww[1], ww[2], ww[3]);
             }
@@ -445,7 +502,7 @@ k_final(const Params p, int* labels, uint32_t* __restrict__ spins_w, Acc* __rest
     // on ONE address serialise in a single L2 slice and stall the whole kernel (measured: 0.71 -> 0.50 ms at beta = 0.5)
     if (threadIdx.x == 0 && sm.ncl)
         atomicAdd(&acc->part[(blockIdx.x + 5 * blockIdx.y) & (ACC_PARTS - 1)].n_clusters, (unsigned long long)sm.ncl);
-    if (MODE == MODE_WOLFF) {
+    if (MODE == MODE_WOLFF || MODE == MODE_FEW) {
         nflip = __reduce_add_sync(FULLM, nflip);
         if (lane == 0 && nflip) atomicAdd(&sm.nflip, nflip);
         __syncthreads();

@@ -789,6 +789,52 @@ int wolff_step(sw_handle* h, int64_t n, int64_t* h_sizes, void* stream)
     return SW_OK;
 }
 
+// n few-cluster steps (label_kernels.cuh: k_few_seeds + k_final<MODE_FEW>): decompose the whole lattice, select the clusters
+// that hold a seed site, flip each selected cluster with probability T_flip / 2^32
+int sw_fewcluster_step(sw_handle* h, int64_t n, int32_t n_seeds, uint32_t T_flip, int64_t* h_flipped, void* stream)
+{
+    if (!h || n < 0 || n_seeds < 0 || n_seeds > 65536) return SW_EINVAL;
+    if (h->q != 2 || h->dim != 2) return SW_EINVAL;      // as wolff_step: defined for the Ising model on the square lattice
+    int slots = 2;
+    while (slots < 2 * n_seeds) slots *= 2;
+    if ((int64_t)slots > h->N) return SW_EINVAL;         // the table of selected roots lives in the N-int cluster-size scratch
+    if (!h->bound || h->nbands > 1) return SW_ESTATE;
+    DeviceGuard guard(h);
+    cudaStream_t s = (cudaStream_t)stream;
+    int64_t done = 0;
+    while (done < n) {
+        const int64_t batch = (n - done) < WOLFF_RING ? (n - done) : WOLFF_RING;
+        SW_CUDA(h, cudaMemsetAsync(h->d_wolff, 0, sizeof(unsigned long long) * (size_t)batch, s));
+        for (int64_t k = 0; k < batch; ++k) {
+            Params p = params_at(h, h->t);
+            p.T_flip = T_flip; p.few_mask = slots - 1;
+            int rc = zero_sweep_counters(h, s);
+            if (rc) return rc;
+            rc = launch_label_front<SRC_PHILOX>(h, p, nullptr, h->d_labels, s, true);
+            if (rc) return rc;
+            k_few_seeds<<<1, 256, 0, s>>>(p, h->d_labels, h->d_size, n_seeds);
+            SW_LAUNCHED(h, "k_few_seeds");
+            if ((p.L % TW) == 0 && (p.L % TH) == 0)
+                k_final<MODE_FEW, 0, true, true><<<dim3(p.ntx, p.nty), FIN_THREADS, 0, s>>>(p, h->d_labels, h->d_spins, h->d_acc,
+                                                                                          h->d_wolff + k, (uint32_t*)h->d_size);
+            else
+                k_final<MODE_FEW, 0, false, true><<<dim3(p.ntx, p.nty), FIN_THREADS, 0, s>>>(p, h->d_labels, h->d_spins, h->d_acc,
+                                                                                           h->d_wolff + k, (uint32_t*)h->d_size);
+            SW_LAUNCHED(h, "k_final<FEW>");
+            SW_PROF(h, 3, s);
+            if (h->prof_on && h->prof_n < PROF_MAX) ++h->prof_n;
+            ++h->t;
+            h->last_labels = h->d_labels;
+        }
+        if (h_flipped) {
+            SW_CUDA(h, cudaMemcpyAsync(h_flipped + done, h->d_wolff, sizeof(int64_t) * (size_t)batch, cudaMemcpyDeviceToHost, s));
+            SW_CUDA(h, cudaStreamSynchronize(s));
+        }
+        done += batch;
+    }
+    return SW_OK;
+}
+
 int sw_wolff_frontier(sw_handle* h, int max_levels)
 {
     if (!h || max_levels < 0 || h->dim != 2) return SW_EINVAL;

@@ -58,6 +58,8 @@ def test_create_validates_arguments(lib):
     obs = binding.sw_obs()
     assert lib.sw_observables(h, C.byref(obs), None) == binding.SW_ESTATE
     assert lib.sw_sweep(h, -1, None) == binding.SW_EINVAL
+    assert lib.sw_fewcluster_step(h, 1, 4, 1, None, None) == binding.SW_ESTATE
+    assert lib.sw_fewcluster_step(h, 1, 70000, 1, None, None) == binding.SW_EINVAL
     # misaligned / NULL buffers, short workspace
     wb = lib.sw_workspace_bytes(64, 2)
     assert lib.sw_bind(h, None, 16, None, 32, wb, None) == binding.SW_EINVAL
