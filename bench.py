@@ -33,9 +33,9 @@ PHASES = ["k_scan", "k_seam", "k_final"]
 # sw_set_threshold as integers: no method arithmetic in the bench
 PERC_THRESHOLD = {0.3: 1288490188, 0.5: 2147483648, 0.7: 3006477107}
 # ncu counters per launch (dram bytes, warp instructions) are NOT constants of this file: they are read from the tracked
-# capture profiles/r02_counters.json, which records the hash of the kernel sources it was taken on; if the sources have
+# capture profiles/r03_counters.json, which records the hash of the kernel sources it was taken on; if the sources have
 # changed since, the fields are reported as null with the reason (ncu_counters below).
-COUNTERS_FILE = os.path.join(ROOT, "profiles", "r02_counters.json")
+COUNTERS_FILE = os.path.join(ROOT, "profiles", "r03_counters.json")
 EQUIL_SWEEPS = 100               # untimed sweeps before the timed region: SURVEY 8(d) "time sweeps 50-200", equilibrium state
 N_SMSP = 148 * 4
 BYTES_PER_SITE_LABEL = 12.25     # sw_label alone = packed bonds 0.25 + 4 + 4 + 4
@@ -60,13 +60,13 @@ def ncu_counters(L: int, beta: float):
         with open(COUNTERS_FILE) as f:
             c = json.load(f)
     except Exception:
-        return None, "none: profiles/r02_counters.json absent"
+        return None, "none: profiles/r03_counters.json absent"
     if c.get("source_sha") != kernel_source_hash():
-        return None, "stale: profiles/r02_counters.json was captured on kernel sources %s, this run has %s" % (
+        return None, "stale: profiles/r03_counters.json was captured on kernel sources %s, this run has %s" % (
             c.get("source_sha"), kernel_source_hash())
     if c.get("L") != L or abs(c.get("beta", -1.0) - beta) > 1e-6:
-        return None, "profiles/r02_counters.json is for L=%s beta=%s" % (c.get("L"), c.get("beta"))
-    return c["kernels"], "profiles/r02_counters.json (ncu --set full, %s, kernel sources %s)" % (c.get("captured"), c.get("source_sha"))
+        return None, "profiles/r03_counters.json is for L=%s beta=%s" % (c.get("L"), c.get("beta"))
+    return c["kernels"], "profiles/r03_counters.json (ncu --set full, %s, kernel sources %s)" % (c.get("captured"), c.get("source_sha"))
 
 
 def beta_c_ising() -> float:
@@ -265,6 +265,13 @@ def per_config_leg(binding, torch, device):
     ms = ev0.elapsed_time(ev1) / 500
     out["configs[4] Wolff steps, 2D Ising L=4096 beta_c (label everything)"] = {
         "ms_per_step": ms, "mean_cluster_sites": sum(sizes) / 500.0, "ns_per_cluster_site": ms * 1e6 / max(1.0, sum(sizes) / 500.0)}
+    # the few-cluster variant on the same lattice: 64 seed points, p_flip = 0.7 (threshold as stored
+    # for percolation p = 0.7: the same integer floor(0.7 2^32))
+    torch.cuda.synchronize(); ev0.record(stream); flipped = lat.fewcluster_step(500, 64, PERC_THRESHOLD[0.7]); ev1.record(stream)
+    torch.cuda.synchronize()
+    ms = ev0.elapsed_time(ev1) / 500
+    out["few-cluster steps (64 seeds, p_flip=0.7), 2D Ising L=4096 beta_c"] = {
+        "ms_per_step": ms, "mean_flipped_sites": sum(flipped) / 500.0, "ns_per_flipped_site": ms * 1e6 / max(1.0, sum(flipped) / 500.0)}
     lat.close()
     L = 16384
     latp = binding.Lattice(L, 2, 0.1, 1, device=device, with_bonds=True)
